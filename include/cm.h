@@ -1,0 +1,124 @@
+/*
+ * cm.h — C ABI of libcm: gravitational potential on nested Cartesian grids by the
+ * convolution method (Vorobyov, McKevitt, Kulikov, Elbakyan, arXiv 2301.06763).
+ *
+ * The problem (Fig. 1; L105-L116, Eq. 9-10; L170-L186, Eq. 14):
+ * `levels` concentric N^3 Cartesian grids, level 0 the coarsest (the paper's m = 1),
+ * level l+1 covering the central half (coarse indices [N/4, 3N/4) per axis, L76) of
+ * level l with cells of half the size, dx_l = dx0 / 2^l.  Given the density rho on
+ * every level, return on every level
+ *
+ *     Phi(Omega^n) = Phi^{m=n} + sum_{k<n} tilde Phi_hole^{m=k}                 (Eq. 14)
+ *
+ * where Phi^m is the discrete sum of Eq. 10 over grid m (masses rho dx^3, inverse
+ * distance between cell centres, the own-cell term of Eq. 13), Phi_hole^m the same
+ * sum with the density inside the cavity set to zero (L174), both evaluated by the
+ * convolution theorem on the zero-padded doubled mesh (Eq. 11), and the
+ * tilde is the coarse->fine interpolation of Eq. 3-6 applied level by level.  The
+ * density a coarse grid sees under a finer grid is the fine density projected onto
+ * it (L280-L282).  DESIGN.md lists every reading of the paper this relies on.
+ *
+ * All entry points return an int status (CM_OK = 0, negative = error); none throws,
+ * aborts or prints.  Pointers are DEVICE pointers unless the name says `host`.
+ * There is no CPU fallback: without a CUDA device every compute call fails with
+ * CM_ECUDA.
+ */
+#ifndef CM_H
+#define CM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cm_plan cm_plan; /* opaque; owned by the library */
+
+enum {
+    CM_OK = 0,
+    CM_EINVAL = -1,    /* bad argument (see each call) */
+    CM_ENOMEM = -2,    /* device or host allocation failed */
+    CM_ECUDA = -3,     /* a CUDA runtime call or kernel failed; see cm_last_cuda_error */
+    CM_ENOTREADY = -4  /* cm_potential before cm_green_precompute */
+};
+
+/*
+ * Create a plan for `levels` nested N^3 grids.
+ *   out        : receives the plan (host pointer to a host pointer).
+ *   N          : cells per axis of every level; power of two, 16 <= N <= 256
+ *                (N % 4 == 0 is the method's own requirement, L76).
+ *   levels     : number of nested grids m >= 1 (at most 32).
+ *   dx0        : cell size of level 0, > 0; dx_l = dx0 / 2^l (L48).
+ *   refinement : must be 2 (the paper fixes the ratio, L42).
+ * Allocates all device workspace (see cm_plan_workspace_bytes) and the twiddle
+ * tables; no kernel runs.  CM_EINVAL / CM_ENOMEM / CM_ECUDA on failure, *out = NULL.
+ */
+int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement);
+
+/*
+ * Step a0 (Eq. 10, 13; L143-L147 Fig. 4): sample the dimensionless kernel
+ * g(o) = 1/|o| on the rearranged doubled mesh (array index a -> offset a if a <= N,
+ * else a - 2N), g(0) = 3 ln(2 + sqrt 3) - pi/2 (Eq. 13 for a cube), transform it and
+ * cache the real spectrum K-hat / (2N)^3 in the plan.  One K-hat serves every level:
+ * Phi^l = -G dx_l^2 (rho * g).  Idempotent; synchronises the device.
+ */
+int cm_green_precompute(cm_plan *plan);
+
+/*
+ * The hot path (steps a1-a8 of DESIGN.md): restriction cascade, pruned (2N)^3 FFT
+ * convolution of every (level, full|hole) field with K-hat, crop, prolongation
+ * cascade and the Eq. 14 sum.
+ *   rho_levels : device, const, [levels][N][N][N] fp64, x fastest, level 0 coarsest,
+ *                16-byte aligned.  Coarse cells under a finer grid are ignored
+ *                (the projected fine density is used instead).
+ *   phi_levels : device, same shape, every cell of every level overwritten.
+ *                Must not alias rho_levels.
+ *   stream     : a cudaStream_t (NULL = legacy default stream).  The call enqueues
+ *                work and returns; no host synchronisation, no host<->device copy.
+ * One solve in flight per plan.  CM_ENOTREADY before cm_green_precompute.
+ */
+int cm_potential(cm_plan *plan, const double *rho_levels, double *phi_levels, void *stream);
+
+/*
+ * Same computation with HOST buffers (pinned memory recommended): copies
+ * rho_host -> device staging, runs cm_potential, copies the result into phi_host
+ * and synchronises `stream` before returning.  Staging buffers belong to the plan
+ * and are allocated on first use.
+ */
+int cm_potential_host(cm_plan *plan, const double *rho_host, double *phi_host, void *stream);
+
+/* Release the plan and everything it owns.  NULL is accepted. */
+int cm_plan_destroy(cm_plan *plan);
+
+/* Gravitational constant used in Phi = -G sum M / r (Eq. 9-10); default 1. */
+int cm_plan_set_G(cm_plan *plan, double G);
+
+/* Device bytes owned by the plan (workspace + K-hat + tables, staging excluded). */
+size_t cm_plan_workspace_bytes(const cm_plan *plan);
+
+/* Number of kernels one cm_potential call launches (nodes of its CUDA graph). */
+int cm_plan_kernel_launches(const cm_plan *plan);
+
+/*
+ * Test/diagnostic access to plan-owned intermediates of the LAST solve, copied
+ * device->device into dst (device, fp64) on `stream`:
+ *   CM_BUF_RESTRICTED : [levels-1][N/2]^3  projected density inside each cavity (a1)
+ *   CM_BUF_HOLE       : [levels][N]^3      ext_l + Phi_hole^l (valid on the cavity
+ *                                           region grown by one cell; a8's input)
+ *   CM_BUF_KHAT       : [2N]^3             cached spectrum, in the library's slot order
+ * n_doubles must equal the buffer's size.  CM_EINVAL otherwise.
+ */
+enum { CM_BUF_RESTRICTED = 0, CM_BUF_HOLE = 1, CM_BUF_KHAT = 2 };
+int cm_debug_copy(cm_plan *plan, int which, double *dst, size_t n_doubles, void *stream);
+
+/* Storage slot -> frequency index along a transformed axis of CM_BUF_KHAT (0 <= slot < 2N). */
+int cm_slot_to_freq(int N, int slot);
+
+const char *cm_error_string(int code);
+/* Text of the last CUDA error seen by this plan ("" if none). */
+const char *cm_last_cuda_error(const cm_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CM_H */

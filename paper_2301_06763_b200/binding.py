@@ -1,0 +1,176 @@
+"""ctypes binding of include/cm.h — argument marshalling only.
+
+Every step of the path runs in libcm's CUDA kernels.  PyTorch supplies device memory
+(`tensor.data_ptr()`) and streams (`torch.cuda.current_stream().cuda_stream`); nothing
+here computes.  If libcm.so is missing or a call fails this raises — there is no
+fallback of any kind.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from functools import lru_cache
+
+from . import _build
+
+CM_OK, CM_EINVAL, CM_ENOMEM, CM_ECUDA, CM_ENOTREADY = 0, -1, -2, -3, -4
+CM_BUF_RESTRICTED, CM_BUF_HOLE, CM_BUF_KHAT = 0, 1, 2
+
+EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potential_host", "cm_plan_destroy",
+           "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
+           "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error"]
+
+
+class CMError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libcm error {code}: {msg}")
+        self.code = code
+
+
+@lru_cache(maxsize=1)
+def lib() -> C.CDLL:
+    if not os.path.exists(_build.SO):
+        raise RuntimeError(f"{_build.SO} is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                           "(no CPU fallback exists)")
+    L = C.CDLL(_build.SO)
+    vp = C.c_void_p
+    L.cm_plan_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_double, C.c_int]
+    L.cm_green_precompute.argtypes = [vp]
+    L.cm_potential.argtypes = [vp, vp, vp, vp]
+    L.cm_potential_host.argtypes = [vp, vp, vp, vp]
+    L.cm_plan_destroy.argtypes = [vp]
+    L.cm_plan_set_G.argtypes = [vp, C.c_double]
+    L.cm_plan_workspace_bytes.argtypes = [vp]
+    L.cm_plan_workspace_bytes.restype = C.c_size_t
+    L.cm_plan_kernel_launches.argtypes = [vp]
+    L.cm_debug_copy.argtypes = [vp, C.c_int, vp, C.c_size_t, vp]
+    L.cm_slot_to_freq.argtypes = [C.c_int, C.c_int]
+    L.cm_error_string.argtypes = [C.c_int]
+    L.cm_error_string.restype = C.c_char_p
+    L.cm_last_cuda_error.argtypes = [vp]
+    L.cm_last_cuda_error.restype = C.c_char_p
+    return L
+
+
+def _check(code: int, plan=None):
+    if code != CM_OK:
+        msg = lib().cm_error_string(code).decode()
+        if plan:
+            extra = lib().cm_last_cuda_error(plan).decode()
+            if extra:
+                msg += " (" + extra + ")"
+        raise CMError(code, msg)
+
+
+# ---- the C ABI, name for name ------------------------------------------------------
+def cm_plan_create(N: int, levels: int, dx0: float, refinement: int = 2) -> int:
+    h = C.c_void_p()
+    _check(lib().cm_plan_create(C.byref(h), int(N), int(levels), float(dx0), int(refinement)))
+    return h.value
+
+
+def cm_green_precompute(plan: int) -> None:
+    _check(lib().cm_green_precompute(plan), plan)
+
+
+def cm_potential(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0) -> None:
+    _check(lib().cm_potential(plan, rho_ptr, phi_ptr, stream), plan)
+
+
+def cm_potential_host(plan: int, rho_host_ptr: int, phi_host_ptr: int, stream: int = 0) -> None:
+    _check(lib().cm_potential_host(plan, rho_host_ptr, phi_host_ptr, stream), plan)
+
+
+def cm_plan_destroy(plan: int) -> None:
+    _check(lib().cm_plan_destroy(plan))
+
+
+def cm_plan_set_G(plan: int, G: float) -> None:
+    _check(lib().cm_plan_set_G(plan, float(G)), plan)
+
+
+def cm_plan_workspace_bytes(plan: int) -> int:
+    return int(lib().cm_plan_workspace_bytes(plan))
+
+
+def cm_plan_kernel_launches(plan: int) -> int:
+    return int(lib().cm_plan_kernel_launches(plan))
+
+
+def cm_debug_copy(plan: int, which: int, dst_ptr: int, n_doubles: int, stream: int = 0) -> None:
+    _check(lib().cm_debug_copy(plan, which, dst_ptr, n_doubles, stream), plan)
+
+
+def cm_slot_to_freq(N: int, slot: int) -> int:
+    return int(lib().cm_slot_to_freq(N, slot))
+
+
+# ---- convenience wrapper over torch tensors (still marshalling only) ---------------
+class Plan:
+    """Owns a cm_plan; `potential` takes/returns CUDA float64 tensors [levels, N, N, N]."""
+
+    def __init__(self, N: int, levels: int, dx0: float, G: float = 1.0, refinement: int = 2):
+        self.N, self.levels, self.dx0 = int(N), int(levels), float(dx0)
+        self._h = cm_plan_create(N, levels, dx0, refinement)
+        if G != 1.0:
+            cm_plan_set_G(self._h, G)
+        cm_green_precompute(self._h)
+
+    @property
+    def handle(self) -> int:
+        return self._h
+
+    def _check_tensor(self, t, device_type):
+        import torch
+        shape = (self.levels, self.N, self.N, self.N)
+        if t.dtype != torch.float64 or tuple(t.shape) != shape or not t.is_contiguous() or t.device.type != device_type:
+            raise ValueError(f"expected contiguous float64 {device_type} tensor of shape {shape}")
+
+    def potential(self, rho, phi=None, stream=None):
+        import torch
+        self._check_tensor(rho, "cuda")
+        if phi is None:
+            phi = torch.empty_like(rho)
+        self._check_tensor(phi, "cuda")
+        s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
+        cm_potential(self._h, rho.data_ptr(), phi.data_ptr(), s)
+        return phi
+
+    def potential_host(self, rho_host, phi_host=None, stream=None):
+        import torch
+        self._check_tensor(rho_host, "cpu")
+        if phi_host is None:
+            phi_host = torch.empty_like(rho_host).pin_memory()
+        self._check_tensor(phi_host, "cpu")
+        s = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
+        cm_potential_host(self._h, rho_host.data_ptr(), phi_host.data_ptr(), s)
+        return phi_host
+
+    def debug_buffer(self, which: int):
+        import torch
+        N, L = self.N, self.levels
+        shape = {CM_BUF_RESTRICTED: (max(L - 1, 0), N // 2, N // 2, N // 2), CM_BUF_HOLE: (L, N, N, N),
+                 CM_BUF_KHAT: (2 * N, 2 * N, 2 * N)}[which]
+        out = torch.empty(shape, dtype=torch.float64, device="cuda")
+        if out.numel():
+            cm_debug_copy(self._h, which, out.data_ptr(), out.numel(), torch.cuda.current_stream().cuda_stream)
+        return out
+
+    @property
+    def workspace_bytes(self) -> int:
+        return cm_plan_workspace_bytes(self._h)
+
+    @property
+    def kernel_launches(self) -> int:
+        return cm_plan_kernel_launches(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            cm_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

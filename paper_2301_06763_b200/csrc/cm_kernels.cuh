@@ -1,0 +1,440 @@
+// cm_kernels.cuh — the CUDA kernels of libcm (sm_100a, fp64).
+//
+// Data flow of one solve (steps a1-a8 of SURVEY.md §8):
+//
+//   rho --k_restrict (fine->coarse cascade)--> rc        projected cavity density (L280-L282)
+//   per level b one COMPLEX field  c_b = rho_full + i rho_hole  (K-hat is real, so the
+//   real/imaginary parts of the convolution are Phi_full and Phi_hole: L174-L176)
+//   P1 k_x_fwd : rho,rc      -> W1[b][z<N][y<N][sx<2N]     x transform of [N data, N zeros]
+//   P2 k_y_fwd : W1          -> W2[b][z<N][sy<2N][sx<2N]
+//   P3 k_z_conv: W2 in place    z transform, * K-hat (Eq. 11), inverse z, keep z < N
+//   P4 k_y_inv : W2          -> W1[b][z<N][y<N][sx<2N]
+//   P5 k_x_inv : W1          -> phi (Re) and hole (Im), scaled by -G dx_b^2, x < N kept
+//   phi,hole --k_prolong_sum (coarse->fine cascade, Eq. 3-6 + Eq. 14)--> phi
+//
+// "sx, sy, sz" are storage slots, not frequencies: slot s = p N + 16 k2 + k1 holds
+// frequency 2 k1 + p + 32 k2 (cm_fft.cuh).  The order is whatever makes every global
+// access a full 128-byte segment; K-hat is stored in the same slot order.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "cm_fft.cuh"
+
+namespace cmk {
+
+using cmfft::cadd;
+using cmfft::cmul;
+using cmfft::cmulc;
+using cmfft::Dft;
+
+constexpr int kThreads = 128;
+
+// ---- compile-time loops over the w_32^r modulation -------------------------------
+template <int R, int DIR> struct ModW32 {
+    __device__ __forceinline__ static void run(double2 *b)
+    {
+        b[R] = cmfft::mulw32<R, DIR>(b[R]);
+        ModW32<R - 1, DIR>::run(b);
+    }
+};
+template <int DIR> struct ModW32<0, DIR> { __device__ __forceinline__ static void run(double2 *) {} };
+
+// ---- shared-memory exchange layouts ----------------------------------------------
+// One pencil's exchange buffer is a [16 (k1)][T (j)] matrix of complex, row stride RS,
+// pencil stride PS (in complex elements).  16-byte accesses: a quarter-warp (8 lanes)
+// must hit 8 distinct 16-byte columns modulo 128 B.
+//  * batch-fastest mapping (y/z passes): the 8 lanes of a quarter-warp are 8 adjacent
+//    pencils with the same j  ->  PS odd.
+//  * j-fastest mapping (x passes): lanes are consecutive j of one row (and, for T < 8,
+//    several rows)  ->  RS odd; PS = 4 (T=4) or 2 (T=2) modulo 8.
+template <int T> struct LayBatch {
+    static constexpr int RS = T;
+    static constexpr int PS = 16 * T + 1;
+};
+template <int T> struct LayRow {
+    static constexpr int RS = T + 1;
+    static constexpr int PS = 16 * (T + 1) + (T == 4 ? 4 : (T == 2 ? 2 : 0));
+};
+
+struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+struct SyncWarp  { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
+
+// ---- half transforms ---------------------------------------------------------------
+// Forward, parity P: a[r] = input element n = j + T r (r < 16).  On return
+// v[cc*T + k2] is the spectrum value of slot  P*N + 16*k2 + cc*T + j.
+template <int T, int P, class Lay, class Sync>
+__device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16], int j, double2 *sm,
+                                         const double2 *__restrict__ tw, Sync sync)
+{
+    double2 b[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) b[r] = a[r];
+    if (P) ModW32<15, -1>::run(b);
+    Dft<16, -1>::run(b);
+    if (T > 1) {
+#pragma unroll
+        for (int k1 = 0; k1 < 16; ++k1) {
+            if (k1 > 0 || P) b[k1] = cmul(b[k1], __ldg(&tw[j * (2 * k1 + P)]));
+            sm[k1 * Lay::RS + j] = b[k1];
+        }
+        sync();
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc) {
+#pragma unroll
+            for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = sm[(cc * T + j) * Lay::RS + jj];
+            Dft<T, -1>::run(&v[cc * T]);
+        }
+    } else {
+#pragma unroll
+        for (int k1 = 0; k1 < 16; ++k1) v[k1] = b[k1];
+    }
+}
+
+// Inverse, parity P: v as above (consumed); on return o[r] is parity P's contribution
+// to output element n = j + T r, r < 16 (the cropped half), already multiplied by
+// conj(w_32^r) for P = 1.
+template <int T, int P, class Lay, class Sync>
+__device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm,
+                                         const double2 *__restrict__ tw, Sync sync)
+{
+    if (T > 1) {
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc) {
+            Dft<T, +1>::run(&v[cc * T]);
+#pragma unroll
+            for (int jj = 0; jj < T; ++jj) sm[(cc * T + j) * Lay::RS + jj] = v[cc * T + jj];
+        }
+        sync();
+#pragma unroll
+        for (int k1 = 0; k1 < 16; ++k1) {
+            o[k1] = sm[k1 * Lay::RS + j];
+            if (k1 > 0 || P) o[k1] = cmulc(o[k1], __ldg(&tw[j * (2 * k1 + P)]));
+        }
+    } else {
+#pragma unroll
+        for (int k1 = 0; k1 < 16; ++k1) o[k1] = v[k1];
+    }
+    Dft<16, +1>::run(o);
+    if (P) ModW32<15, +1>::run(o);
+}
+
+__device__ __forceinline__ bool in_cavity1(int v, int N) { return v >= N / 4 && v < 3 * N / 4; }
+__device__ __forceinline__ bool in_ring1(int v, int N) { return v >= N / 4 - 1 && v <= 3 * N / 4; }
+
+// ================================ P1: x forward ====================================
+// One row (b, z, y) per group of T threads (j fastest).  Reads N reals, forms the complex
+// pair field (step a2, never materialised), writes 2N complex slots.
+template <int T>
+__global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ rho, const double *__restrict__ rc,
+                                                    double2 *__restrict__ W1, const double2 *__restrict__ tw, int L)
+{
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, H = N / 2, Q = N / 4;
+    using Lay = LayRow<T>;
+    extern __shared__ double2 smem[];
+    const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
+    const size_t row = (size_t)blockIdx.x * ROWS + rowl;
+    const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
+    const bool finest = (b == L - 1);
+    const bool rowcav = !finest && in_cavity1(z, N) && in_cavity1(y, N);
+    const double *src = rho + row * N;
+    const double *srcc = rowcav ? rc + (((size_t)b * H + (z - Q)) * H + (y - Q)) * H - Q : rho;
+
+    double2 a[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int x = j + T * r;
+        const bool cav = rowcav && in_cavity1(x, N);
+        const double re = cav ? __ldg(srcc + x) : __ldg(src + x);
+        a[r] = make_double2(re, (finest || cav) ? 0.0 : re);
+    }
+    double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
+    double2 *dst = W1 + row * NN;
+    {
+        double2 v[16];
+        fwd_half<T, 0, Lay>(a, v, j, bufA, tw, SyncWarp());
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+            for (int k2 = 0; k2 < T; ++k2) dst[16 * k2 + cc * T + j] = v[cc * T + k2];
+    }
+    {
+        double2 v[16];
+        fwd_half<T, 1, Lay>(a, v, j, bufB, tw, SyncWarp());
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+            for (int k2 = 0; k2 < T; ++k2) dst[N + 16 * k2 + cc * T + j] = v[cc * T + k2];
+    }
+}
+
+// ================================ P5: x inverse ====================================
+template <int T>
+__global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
+                                                    double *__restrict__ hole, const double2 *__restrict__ tw,
+                                                    int L, double scale0 /* -G dx0^2 */)
+{
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T;
+    using Lay = LayRow<T>;
+    extern __shared__ double2 smem[];
+    const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
+    const size_t row = (size_t)blockIdx.x * ROWS + rowl;
+    const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
+    const double2 *src = W1 + row * NN;
+    double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
+
+    double2 v0[16], v1[16];
+#pragma unroll
+    for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+        for (int k2 = 0; k2 < T; ++k2) {
+            v0[cc * T + k2] = src[16 * k2 + cc * T + j];
+            v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
+        }
+    double2 e[16], o[16];
+    inv_half<T, 0, Lay>(v0, e, j, bufA, tw, SyncWarp());
+    inv_half<T, 1, Lay>(v1, o, j, bufB, tw, SyncWarp());
+
+    const double scale = scale0 * exp2(-2.0 * b);   // dx_b^2 = dx0^2 / 4^b, exact
+    const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
+    double *dphi = phi + row * N, *dh = hole + row * N;
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int x = j + T * r;
+        dphi[x] = scale * (e[r].x + o[r].x);
+        if (rowring && in_ring1(x, N)) dh[x] = scale * (e[r].y + o[r].y);
+    }
+}
+
+// ======================= batch-fastest mapping (y and z passes) ====================
+// tid -> px = tid & 7 (8 adjacent slots = one 128-byte segment), j = (tid >> 3) % T,
+// g = tid / (8 T).  A CTA covers 8 * G adjacent batch positions, G = 16 / T.
+
+// ================================ P2: y forward ====================================
+template <int T>
+__global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ W1, double2 *__restrict__ W2,
+                                                    const double2 *__restrict__ tw)
+{
+    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    using Lay = LayBatch<T>;
+    extern __shared__ double2 smem[];
+    const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
+    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
+    const size_t bz = q / NN;
+    const int sx = (int)(q % NN);
+    const double2 *src = W1 + bz * N * NN + sx;
+    double2 *dst = W2 + bz * NN * NN + sx;
+    double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
+
+    double2 a[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) a[r] = src[(size_t)(j + T * r) * NN];
+    {
+        double2 v[16];
+        fwd_half<T, 0, Lay>(a, v, j, bufA, tw, SyncBlock());
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+            for (int k2 = 0; k2 < T; ++k2) dst[(size_t)(16 * k2 + cc * T + j) * NN] = v[cc * T + k2];
+    }
+    {
+        double2 v[16];
+        fwd_half<T, 1, Lay>(a, v, j, bufB, tw, SyncBlock());
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+            for (int k2 = 0; k2 < T; ++k2) dst[(size_t)(N + 16 * k2 + cc * T + j) * NN] = v[cc * T + k2];
+    }
+}
+
+// ================================ P4: y inverse ====================================
+template <int T>
+__global__ void __launch_bounds__(kThreads) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
+                                                    const double2 *__restrict__ tw)
+{
+    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    using Lay = LayBatch<T>;
+    extern __shared__ double2 smem[];
+    const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
+    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;
+    const size_t bz = q / NN;
+    const int sx = (int)(q % NN);
+    const double2 *src = W2 + bz * NN * NN + sx;
+    double2 *dst = W1 + bz * N * NN + sx;
+    double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
+
+    double2 v0[16], v1[16];
+#pragma unroll
+    for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+        for (int k2 = 0; k2 < T; ++k2) {
+            v0[cc * T + k2] = src[(size_t)(16 * k2 + cc * T + j) * NN];
+            v1[cc * T + k2] = src[(size_t)(N + 16 * k2 + cc * T + j) * NN];
+        }
+    double2 e[16], o[16];
+    inv_half<T, 0, Lay>(v0, e, j, bufA, tw, SyncBlock());
+    inv_half<T, 1, Lay>(v1, o, j, bufB, tw, SyncBlock());
+#pragma unroll
+    for (int r = 0; r < 16; ++r) dst[(size_t)(j + T * r) * NN] = cadd(e[r], o[r]);
+}
+
+// ====================== P3: z forward * K-hat * z inverse ==========================
+// blockIdx.x = tile * L + b: the L levels that share one K-hat tile run together so
+// the tile comes from HBM once and from L2 afterwards.
+template <int T>
+__global__ void __launch_bounds__(kThreads) k_z_conv(double2 *__restrict__ W2, const double *__restrict__ Khat,
+                                                     const double2 *__restrict__ tw, int L)
+{
+    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    using Lay = LayBatch<T>;
+    extern __shared__ double2 smem[];
+    const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
+    const int b = blockIdx.x % L;
+    const size_t flat = (size_t)(blockIdx.x / L) * PEN + g * 8 + px;   // sy * 2N + sx
+    const size_t zs = (size_t)NN * NN;
+    double2 *base = W2 + (size_t)b * N * zs + flat;
+    const double *kh = Khat + flat;
+    double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
+
+    double2 a[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) a[r] = base[(size_t)(j + T * r) * zs];
+
+    double2 e[16];
+    {
+        double2 v[16];
+        fwd_half<T, 0, Lay>(a, v, j, bufA, tw, SyncBlock());
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+            for (int k2 = 0; k2 < T; ++k2) {
+                const double k = __ldg(kh + (size_t)(16 * k2 + cc * T + j) * zs);
+                v[cc * T + k2].x *= k;
+                v[cc * T + k2].y *= k;
+            }
+        inv_half<T, 0, Lay>(v, e, j, bufB, tw, SyncBlock());
+    }
+    {
+        double2 v[16], o[16];
+        fwd_half<T, 1, Lay>(a, v, j, bufA, tw, SyncBlock());
+#pragma unroll
+        for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+            for (int k2 = 0; k2 < T; ++k2) {
+                const double k = __ldg(kh + (size_t)(N + 16 * k2 + cc * T + j) * zs);
+                v[cc * T + k2].x *= k;
+                v[cc * T + k2].y *= k;
+            }
+        inv_half<T, 1, Lay>(v, o, j, bufB, tw, SyncBlock());
+#pragma unroll
+        for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
+    }
+#pragma unroll
+    for (int r = 0; r < 16; ++r) base[(size_t)(j + T * r) * zs] = e[r];
+}
+
+// ============================ a1: restriction cascade ==============================
+// rc[lf-1][ck][cj][ci] = mean of the 8 children of fine level lf, where a child that lies
+// under level lf+1 takes the already projected value rc[lf] (L280-L282; readings 9, 10).
+__global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_f, const double *__restrict__ rc_f,
+                           double *__restrict__ rc_out)
+{
+    const int H = N / 2, Q = N / 4;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= H * H * H) return;
+    const int ci = idx % H, cj = (idx / H) % H, ck = idx / (H * H);
+    const bool use_rc = (lf < L - 1);
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+            for (int a = 0; a < 2; ++a) {
+                const int k = 2 * ck + c, jx = 2 * cj + bb, i = 2 * ci + a;
+                const bool cav = use_rc && in_cavity1(k, N) && in_cavity1(jx, N) && in_cavity1(i, N);
+                s += cav ? rc_f[((size_t)(k - Q) * H + (jx - Q)) * H + (i - Q)]
+                         : rho_f[((size_t)k * N + jx) * N + i];
+            }
+    rc_out[idx] = 0.125 * s;
+}
+
+// ===================== a8: prolongation + Eq. 14 sum, one level ====================
+// Hc = ext_{l-1} + Phi_hole^{l-1} on the coarse grid (valid on the cavity grown by one
+// cell).  Fine cell f: parent p = N/4 + f/2, sign s = +1 (f odd) / -1 (f even);
+// ext_l(f) = 3/4 Hc[p] + 1/4 Hc[p+s]  (Eq. 3-6); phi_l += ext_l  (Eq. 14);
+// hole_l += ext_l where the next level will need it.
+__global__ void k_prolong_sum(int N, int l, int L, const double *__restrict__ Hc, double *__restrict__ phi_l,
+                              double *__restrict__ hole_l)
+{
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= N * N * N) return;
+    const int fi = idx % N, fj = (idx / N) % N, fk = idx / (N * N);
+    const int Q = N / 4;
+    const int pk = Q + fk / 2, pj = Q + fj / 2, pi = Q + fi / 2;
+    const int sk = (fk & 1) ? 1 : -1, sj = (fj & 1) ? 1 : -1, si = (fi & 1) ? 1 : -1;
+    const double e = 0.75 * Hc[((size_t)pk * N + pj) * N + pi] +
+                     0.25 * Hc[((size_t)(pk + sk) * N + (pj + sj)) * N + (pi + si)];
+    phi_l[idx] += e;
+    if (l < L - 1 && in_ring1(fk, N) && in_ring1(fj, N) && in_ring1(fi, N)) hole_l[idx] += e;
+}
+
+// ============================ a0: Green's function ================================
+// g on the rearranged doubled mesh (Fig. 4): index a -> offset a (a <= N) or a - 2N.
+__global__ void k_green_sample(double2 *__restrict__ Gm, int N, double I0)
+{
+    const int n = 2 * N;
+    const size_t tot = (size_t)n * n * n;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < tot; q += (size_t)gridDim.x * blockDim.x) {
+        const int a = (int)(q % n), bb = (int)((q / n) % n), c = (int)(q / ((size_t)n * n));
+        const double ox = a <= N ? a : a - n, oy = bb <= N ? bb : bb - n, oz = c <= N ? c : c - n;
+        const double d2 = ox * ox + oy * oy + oz * oz;
+        Gm[q] = make_double2(d2 == 0.0 ? I0 : 1.0 / sqrt(d2), 0.0);
+    }
+}
+
+// Plain in-place radix-2 transform of one pencil per CTA (one-time set-up, not the hot
+// path): n = 2N points, n/2 threads, natural order in and out.
+__global__ void k_fft_simple(double2 *__restrict__ data, int n, int log2n, int axis, const double2 *__restrict__ tw)
+{
+    extern __shared__ double2 sm[];
+    const size_t u = blockIdx.x / n, v = blockIdx.x % n;
+    size_t base, stride;
+    if (axis == 0) { base = (u * n + v) * n; stride = 1; }
+    else if (axis == 1) { base = u * n * n + v; stride = n; }
+    else { base = u * n + v; stride = (size_t)n * n; }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const int rev = (int)(__brev((unsigned)i) >> (32 - log2n));
+        sm[rev] = data[base + (size_t)i * stride];
+    }
+    __syncthreads();
+    for (int len = 2; len <= n; len <<= 1) {
+        const int half = len >> 1, step = n / len;
+        for (int t = threadIdx.x; t < n / 2; t += blockDim.x) {
+            const int grp = t / half, k = t % half;
+            const int i0 = grp * len + k, i1 = i0 + half;
+            const double2 w = tw[k * step];
+            const double2 x0 = sm[i0], x1 = cmul(sm[i1], w);
+            sm[i0] = cadd(x0, x1);
+            sm[i1] = cmfft::csub(x0, x1);
+        }
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) data[base + (size_t)i * stride] = sm[i];
+}
+
+// K-hat[sz][sy][sx] = Re Ghat[f(sz)][f(sy)][f(sx)] / (2N)^3, f = slot_to_freq.
+__global__ void k_green_permute(const double2 *__restrict__ Gm, double *__restrict__ Khat, int N)
+{
+    const int n = 2 * N;
+    const size_t tot = (size_t)n * n * n;
+    const double inv = 1.0 / ((double)n * (double)n * (double)n);
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < tot; q += (size_t)gridDim.x * blockDim.x) {
+        const int sx = (int)(q % n), sy = (int)((q / n) % n), sz = (int)(q / ((size_t)n * n));
+        const size_t fx = cmfft::slot_to_freq(sx, N), fy = cmfft::slot_to_freq(sy, N), fz = cmfft::slot_to_freq(sz, N);
+        Khat[q] = Gm[(fz * n + fy) * n + fx].x * inv;
+    }
+}
+
+}  // namespace cmk

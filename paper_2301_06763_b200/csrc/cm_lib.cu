@@ -1,0 +1,363 @@
+// cm_lib.cu — the C ABI of include/cm.h: plan, workspace, CUDA-graph capture.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/cm.h"
+#include "cm_kernels.cuh"
+
+namespace {
+
+struct GraphEntry {
+    const double *rho;
+    double *phi;
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+};
+
+}  // namespace
+
+struct cm_plan {
+    int N = 0, L = 0, T = 0;
+    double dx0 = 0, G = 1.0;
+    double2 *W1 = nullptr, *W2 = nullptr, *tw = nullptr;
+    double *Khat = nullptr, *rc = nullptr, *hole = nullptr;
+    double *stage_rho = nullptr, *stage_phi = nullptr;
+    size_t bytes = 0;
+    bool green_ready = false;
+    bool use_graph = true;
+    cudaStream_t cap_stream = nullptr;
+    std::vector<GraphEntry> graphs;
+    int launches = 0;
+    char err[512] = {0};
+};
+
+namespace {
+
+using namespace cmk;
+
+bool cuda_fail(cm_plan *p, cudaError_t e, const char *what)
+{
+    if (e == cudaSuccess) return false;
+    if (p) std::snprintf(p->err, sizeof(p->err), "%s: %s", what, cudaGetErrorString(e));
+    return true;
+}
+#define CM_CUDA(p, call)                                  \
+    do {                                                  \
+        if (cuda_fail((p), (call), #call)) return CM_ECUDA; \
+    } while (0)
+
+template <int T> size_t smem_row() { return sizeof(double2) * 2 * (kThreads / T) * LayRow<T>::PS; }
+template <int T> size_t smem_batch() { return sizeof(double2) * 2 * (8 * (16 / T)) * LayBatch<T>::PS; }
+
+template <int T> int set_attrs(cm_plan *p)
+{
+    CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_z_conv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    return CM_OK;
+}
+
+// The five FFT passes for every level at once (steps a3-a7).
+template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s)
+{
+    constexpr int N = 16 * T, NN = 2 * N;
+    const int L = p->L;
+    const size_t rows = (size_t)L * N * N;
+    const unsigned gx = (unsigned)(rows / (kThreads / T));
+    const unsigned gy = (unsigned)((size_t)L * N * NN / (8 * (16 / T)));
+    const unsigned gz = (unsigned)((size_t)NN * NN / (8 * (16 / T)) * L);
+    k_x_fwd<T><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
+    k_y_fwd<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    k_z_conv<T><<<gz, kThreads, smem_batch<T>(), s>>>(p->W2, p->Khat, p->tw, L);
+    k_y_inv<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
+    k_x_inv<T><<<gx, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->tw, L, -p->G * p->dx0 * p->dx0);
+    p->launches += 5;
+    CM_CUDA(p, cudaGetLastError());
+    return CM_OK;
+}
+
+int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s)
+{
+    const int N = p->N, L = p->L, H = N / 2;
+    const size_t n3 = (size_t)N * N * N, h3 = (size_t)H * H * H;
+    p->launches = 0;
+    // a1: restriction cascade, fine -> coarse
+    for (int lf = L - 1; lf >= 1; --lf) {
+        const double *rc_f = (lf < L - 1) ? p->rc + h3 * lf : nullptr;
+        k_restrict<<<(unsigned)((h3 + 255) / 256), 256, 0, s>>>(N, lf, L, rho + n3 * lf, rc_f, p->rc + h3 * (lf - 1));
+        p->launches++;
+    }
+    CM_CUDA(p, cudaGetLastError());
+    int rcode = CM_EINVAL;
+    switch (p->T) {
+        case 1: rcode = launch_passes<1>(p, rho, phi, s); break;
+        case 2: rcode = launch_passes<2>(p, rho, phi, s); break;
+        case 4: rcode = launch_passes<4>(p, rho, phi, s); break;
+        case 8: rcode = launch_passes<8>(p, rho, phi, s); break;
+        case 16: rcode = launch_passes<16>(p, rho, phi, s); break;
+    }
+    if (rcode != CM_OK) return rcode;
+    // a8: prolongation + Eq. 14 sum, coarse -> fine
+    for (int l = 1; l < L; ++l) {
+        k_prolong_sum<<<(unsigned)((n3 + 255) / 256), 256, 0, s>>>(N, l, L, p->hole + n3 * (l - 1), phi + n3 * l,
+                                                                    p->hole + n3 * l);
+        p->launches++;
+    }
+    CM_CUDA(p, cudaGetLastError());
+    return CM_OK;
+}
+
+void destroy_graphs(cm_plan *p)
+{
+    for (auto &g : p->graphs) {
+        if (g.exec) cudaGraphExecDestroy(g.exec);
+        if (g.graph) cudaGraphDestroy(g.graph);
+    }
+    p->graphs.clear();
+}
+
+template <class Tp> int dev_alloc(cm_plan *p, Tp **ptr, size_t count)
+{
+    void *q = nullptr;
+    cudaError_t e = cudaMalloc(&q, count * sizeof(Tp));
+    if (e == cudaErrorMemoryAllocation) {
+        cuda_fail(p, e, "cudaMalloc");
+        cudaGetLastError();
+        return CM_ENOMEM;
+    }
+    if (cuda_fail(p, e, "cudaMalloc")) return CM_ECUDA;
+    *ptr = (Tp *)q;
+    p->bytes += count * sizeof(Tp);
+    return CM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
+{
+    if (!out) return CM_EINVAL;
+    *out = nullptr;
+    if (refinement != 2) return CM_EINVAL;
+    if (N < 16 || N > 256 || (N & (N - 1)) != 0) return CM_EINVAL;
+    if (levels < 1 || levels > 32) return CM_EINVAL;
+    if (!(dx0 > 0.0) || !std::isfinite(dx0)) return CM_EINVAL;
+
+    cm_plan *p = new (std::nothrow) cm_plan();
+    if (!p) return CM_ENOMEM;
+    p->N = N;
+    p->L = levels;
+    p->T = N / 16;
+    p->dx0 = dx0;
+    const char *ng = std::getenv("CM_NO_GRAPH");
+    p->use_graph = !(ng && ng[0] == '1');
+
+    const size_t n = 2 * (size_t)N, n3 = (size_t)N * N * N, h3 = n3 / 8, L = (size_t)levels;
+    int rc = CM_OK;
+    int ndev = 0;
+    if (cuda_fail(p, cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev == 0) {
+        delete p;
+        return CM_ECUDA;
+    }
+    if ((rc = dev_alloc(p, &p->W1, L * N * N * n)) == CM_OK &&
+        (rc = dev_alloc(p, &p->W2, L * N * n * n)) == CM_OK &&
+        (rc = dev_alloc(p, &p->Khat, n * n * n)) == CM_OK &&
+        (rc = dev_alloc(p, &p->rc, (L > 1 ? L - 1 : 1) * h3)) == CM_OK &&
+        (rc = dev_alloc(p, &p->hole, L * n3)) == CM_OK &&
+        (rc = dev_alloc(p, &p->tw, n)) == CM_OK) {
+        // twiddles w_2N^m = exp(-2 pi i m / 2N), computed in long double on the host
+        std::vector<double2> tw(n);
+        const long double tau = 2.0L * acosl(-1.0L);
+        for (size_t m = 0; m < n; ++m) {
+            const long double a = -tau * (long double)m / (long double)n;
+            tw[m] = make_double2((double)cosl(a), (double)sinl(a));
+        }
+        // exact values on the axes
+        tw[0] = make_double2(1.0, 0.0);
+        tw[n / 4] = make_double2(0.0, -1.0);
+        tw[n / 2] = make_double2(-1.0, 0.0);
+        tw[3 * n / 4] = make_double2(0.0, 1.0);
+        if (cuda_fail(p, cudaMemcpy(p->tw, tw.data(), n * sizeof(double2), cudaMemcpyHostToDevice), "cudaMemcpy(tw)"))
+            rc = CM_ECUDA;
+        else if (cuda_fail(p, cudaMemset(p->hole, 0, L * n3 * sizeof(double)), "cudaMemset")) rc = CM_ECUDA;
+        else if (cuda_fail(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking), "cudaStreamCreate"))
+            rc = CM_ECUDA;
+    }
+    if (rc == CM_OK) {
+        switch (p->T) {
+            case 1: rc = set_attrs<1>(p); break;
+            case 2: rc = set_attrs<2>(p); break;
+            case 4: rc = set_attrs<4>(p); break;
+            case 8: rc = set_attrs<8>(p); break;
+            case 16: rc = set_attrs<16>(p); break;
+        }
+    }
+    if (rc != CM_OK) {
+        cm_plan_destroy(p);
+        return rc;
+    }
+    // number of kernels per solve: (L-1) restrictions + 5 passes + (L-1) prolongations
+    p->launches = 2 * (levels - 1) + 5;
+    *out = p;
+    return CM_OK;
+}
+
+int cm_green_precompute(cm_plan *p)
+{
+    if (!p) return CM_EINVAL;
+    if (p->green_ready) return CM_OK;
+    const int N = p->N, n = 2 * N;
+    const size_t tot = (size_t)n * n * n;
+    double2 *Gm = nullptr;
+    cudaError_t e = cudaMalloc((void **)&Gm, tot * sizeof(double2));
+    if (e != cudaSuccess) {
+        cuda_fail(p, e, "cudaMalloc(green scratch)");
+        cudaGetLastError();
+        return e == cudaErrorMemoryAllocation ? CM_ENOMEM : CM_ECUDA;
+    }
+    const double I0 = (double)(3.0L * logl(2.0L + sqrtl(3.0L)) - acosl(-1.0L) / 2.0L);  // Eq. 13, cube
+    int log2n = 0;
+    while ((1 << log2n) < n) ++log2n;
+    cudaStream_t s = p->cap_stream;
+    k_green_sample<<<1024, 256, 0, s>>>(Gm, N, I0);
+    for (int axis = 0; axis < 3; ++axis)
+        k_fft_simple<<<(unsigned)(n * n), n / 2 < 256 ? n / 2 : 256, n * sizeof(double2), s>>>(Gm, n, log2n, axis, p->tw);
+    k_green_permute<<<1024, 256, 0, s>>>(Gm, p->Khat, N);
+    cudaError_t e1 = cudaGetLastError();
+    cudaError_t e2 = cudaStreamSynchronize(s);
+    cudaFree(Gm);
+    if (cuda_fail(p, e1, "green kernels") || cuda_fail(p, e2, "green sync")) return CM_ECUDA;
+    p->green_ready = true;
+    return CM_OK;
+}
+
+int cm_potential(cm_plan *p, const double *rho, double *phi, void *stream)
+{
+    if (!p || !rho || !phi) return CM_EINVAL;
+    if (((uintptr_t)rho & 15) || ((uintptr_t)phi & 15)) return CM_EINVAL;
+    if (!p->green_ready) return CM_ENOTREADY;
+    const size_t tot = (size_t)p->L * p->N * p->N * p->N;
+    if ((rho <= phi && phi < rho + tot) || (phi <= rho && rho < phi + tot)) return CM_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!p->use_graph) return enqueue_solve(p, rho, phi, s);
+
+    for (auto &g : p->graphs)
+        if (g.rho == rho && g.phi == phi) {
+            CM_CUDA(p, cudaGraphLaunch(g.exec, s));
+            return CM_OK;
+        }
+    // capture once per (rho, phi) pair on the plan's own stream, launch on the caller's
+    GraphEntry ge{rho, phi, nullptr, nullptr};
+    CM_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
+    const int rc = enqueue_solve(p, rho, phi, p->cap_stream);
+    cudaError_t ee = cudaStreamEndCapture(p->cap_stream, &ge.graph);
+    if (rc != CM_OK) {
+        if (ge.graph) cudaGraphDestroy(ge.graph);
+        return rc;
+    }
+    CM_CUDA(p, ee);
+    CM_CUDA(p, cudaGraphInstantiate(&ge.exec, ge.graph, 0));
+    if (p->graphs.size() >= 8) destroy_graphs(p);
+    p->graphs.push_back(ge);
+    CM_CUDA(p, cudaGraphLaunch(ge.exec, s));
+    return CM_OK;
+}
+
+int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void *stream)
+{
+    if (!p || !rho_host || !phi_host) return CM_EINVAL;
+    if (!p->green_ready) return CM_ENOTREADY;
+    const size_t tot = (size_t)p->L * p->N * p->N * p->N;
+    if (!p->stage_rho) {
+        size_t keep = p->bytes;
+        int rc = dev_alloc(p, &p->stage_rho, tot);
+        if (rc == CM_OK) rc = dev_alloc(p, &p->stage_phi, tot);
+        p->bytes = keep;  // staging is reported separately
+        if (rc != CM_OK) return rc;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    CM_CUDA(p, cudaMemcpyAsync(p->stage_rho, rho_host, tot * sizeof(double), cudaMemcpyHostToDevice, s));
+    const int rc = cm_potential(p, p->stage_rho, p->stage_phi, stream);
+    if (rc != CM_OK) return rc;
+    CM_CUDA(p, cudaMemcpyAsync(phi_host, p->stage_phi, tot * sizeof(double), cudaMemcpyDeviceToHost, s));
+    CM_CUDA(p, cudaStreamSynchronize(s));
+    return CM_OK;
+}
+
+int cm_plan_destroy(cm_plan *p)
+{
+    if (!p) return CM_OK;
+    destroy_graphs(p);
+    if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
+    cudaFree(p->W1);
+    cudaFree(p->W2);
+    cudaFree(p->Khat);
+    cudaFree(p->rc);
+    cudaFree(p->hole);
+    cudaFree(p->tw);
+    cudaFree(p->stage_rho);
+    cudaFree(p->stage_phi);
+    delete p;
+    return CM_OK;
+}
+
+int cm_plan_set_G(cm_plan *p, double G)
+{
+    if (!p || !std::isfinite(G)) return CM_EINVAL;
+    if (G != p->G) destroy_graphs(p);  // the scale is baked into the captured kernel arguments
+    p->G = G;
+    return CM_OK;
+}
+
+size_t cm_plan_workspace_bytes(const cm_plan *p) { return p ? p->bytes : 0; }
+
+int cm_plan_kernel_launches(const cm_plan *p) { return p ? 2 * (p->L - 1) + 5 : 0; }
+
+int cm_debug_copy(cm_plan *p, int which, double *dst, size_t n_doubles, void *stream)
+{
+    if (!p || !dst) return CM_EINVAL;
+    const size_t N = p->N, n3 = N * N * N, L = p->L;
+    const double *src = nullptr;
+    size_t cnt = 0;
+    switch (which) {
+        case CM_BUF_RESTRICTED: src = p->rc; cnt = (L - 1) * (n3 / 8); break;
+        case CM_BUF_HOLE: src = p->hole; cnt = L * n3; break;
+        case CM_BUF_KHAT: src = p->Khat; cnt = 8 * n3; break;
+        default: return CM_EINVAL;
+    }
+    if (cnt != n_doubles) return CM_EINVAL;
+    if (cnt == 0) return CM_OK;
+    CM_CUDA(p, cudaMemcpyAsync(dst, src, cnt * sizeof(double), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return CM_OK;
+}
+
+int cm_slot_to_freq(int N, int slot)
+{
+    if (N < 16 || slot < 0 || slot >= 2 * N) return CM_EINVAL;
+    return cmfft::slot_to_freq(slot, N);
+}
+
+const char *cm_error_string(int code)
+{
+    switch (code) {
+        case CM_OK: return "ok";
+        case CM_EINVAL: return "invalid argument";
+        case CM_ENOMEM: return "out of memory";
+        case CM_ECUDA: return "CUDA error";
+        case CM_ENOTREADY: return "cm_green_precompute has not been called";
+        default: return "unknown error";
+    }
+}
+
+const char *cm_last_cuda_error(const cm_plan *p) { return p ? p->err : ""; }
+
+}  // extern "C"

@@ -1,0 +1,274 @@
+"""Parity of the CUDA path (through the C ABI) against the oracle, element by element.
+
+Bar (BASELINE.json north_star): max |phi_gpu - phi_oracle| / max |phi| <= 1e-11 in fp64,
+evaluated per level (the stricter normalisation) and globally.
+"""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def _pkg():
+    import paper_2301_06763_b200 as pkg
+    pkg.build()
+    return pkg
+
+
+def _solve_gpu(rho, dx0, G=1.0):
+    pkg = _pkg()
+    L, N = rho.shape[0], rho.shape[1]
+    plan = pkg.Plan(N, L, dx0, G=G)
+    d_rho = torch.from_numpy(rho).cuda()
+    keep = d_rho.clone()
+    phi = plan.potential(d_rho)
+    torch.cuda.synchronize()
+    assert torch.equal(d_rho, keep), "rho_levels must not be written"
+    out = phi.cpu().numpy()
+    return out, plan
+
+
+def _assert_parity(got, ref, tol=TOL):
+    worst = 0.0
+    for l in range(ref.shape[0]):
+        e = np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()
+        worst = max(worst, e)
+        assert e <= tol, f"level {l}: rel err {e:.3e} > {tol}"
+    assert np.abs(got - ref).max() / np.abs(ref).max() <= tol
+    return worst
+
+
+# ---------------------------------------------------------------- component parity
+@pytest.mark.parametrize("N", [16, 32, 64])
+def test_khat_matches_oracle_green_hat(N):
+    """Step a0: cached spectrum == oracle's transform of the rearranged kernel / (2N)^3,
+    after undoing the library's slot order (cm_slot_to_freq)."""
+    pkg = _pkg()
+    plan = pkg.Plan(N, 1, 1.0)
+    kh = plan.debug_buffer(pkg.CM_BUF_KHAT).cpu().numpy()
+    f = np.array([pkg.cm_slot_to_freq(N, s) for s in range(2 * N)])
+    assert sorted(f.tolist()) == list(range(2 * N))
+    ref = oracle.green_hat(N).real / (2.0 * N) ** 3
+    ref = ref[np.ix_(f, f, f)]
+    assert np.abs(kh - ref).max() <= 1e-13 * np.abs(ref).max()
+    plan.close()
+
+
+def test_restriction_cascade_matches_oracle():
+    pkg = _pkg()
+    N, L = 16, 4
+    rng = np.random.default_rng(3)
+    rho = rng.random((L, N, N, N)) * (4.0 ** np.arange(L))[:, None, None, None]
+    _, plan = _solve_gpu(rho, 0.125)
+    rc = plan.debug_buffer(pkg.CM_BUF_RESTRICTED).cpu().numpy()
+    rb = oracle.restrict(rho)
+    lo, hi = N // 4, 3 * N // 4
+    for l in range(L - 1):
+        assert np.abs(rc[l] - rb[l][lo:hi, lo:hi, lo:hi]).max() <= 1e-15 * np.abs(rb[l]).max()
+    plan.close()
+
+
+def test_hole_plus_ext_buffer_matches_oracle():
+    """a8's input H_l = ext_l + Phi_hole^l on the cavity grown by one cell."""
+    pkg = _pkg()
+    N, L = 16, 3
+    rng = np.random.default_rng(4)
+    rho = rng.random((L, N, N, N))
+    _, plan = _solve_gpu(rho, 0.125)
+    H = plan.debug_buffer(pkg.CM_BUF_HOLE).cpu().numpy()
+    _, parts = oracle.solve(rho, 0.125, method="fft", return_parts=True)
+    lo, hi = N // 4 - 1, 3 * N // 4 + 1
+    for l in range(L - 1):
+        ref = (parts["ext"][l] + parts["hole"][l])[lo:hi, lo:hi, lo:hi]
+        assert np.abs(H[l][lo:hi, lo:hi, lo:hi] - ref).max() <= TOL * np.abs(ref).max()
+    plan.close()
+
+
+# ---------------------------------------------------------------- single level, every supported N
+@pytest.mark.parametrize("N", [16, 32, 64, 128])
+def test_single_level_random_field(N):
+    rng = np.random.default_rng(N)
+    rho = rng.standard_normal((1, N, N, N))
+    got, plan = _solve_gpu(rho, 0.3)
+    ref = oracle.solve(rho, 0.3, method="fft")
+    _assert_parity(got, ref)
+    plan.close()
+
+
+@pytest.mark.parametrize("src", [(0, 0, 0), (15, 15, 15), (15, 0, 7), (3, 9, 15)])
+def test_point_source_closed_form(src):
+    """GPU path against the closed form directly (Eq. 10 / Eq. 13), no oracle involved."""
+    N, dx, G, rho0 = 16, 0.37, 1.7, 2.5
+    rho = np.zeros((1, N, N, N))
+    rho[0][src] = rho0
+    got, plan = _solve_gpu(rho, dx, G=G)
+    k, j, i = np.meshgrid(np.arange(N), np.arange(N), np.arange(N), indexing="ij")
+    d = np.sqrt((k - src[0]) ** 2.0 + (j - src[1]) ** 2.0 + (i - src[2]) ** 2.0)
+    with np.errstate(divide="ignore"):
+        ref = -G * rho0 * dx * dx / d
+    ref[src] = -G * rho0 * dx * dx * (3 * np.log(2 + np.sqrt(3)) - np.pi / 2)
+    assert np.abs(got[0] - ref).max() <= 1e-12 * np.abs(ref).max()
+    plan.close()
+
+
+# ---------------------------------------------------------------- nested, random, ragged sizes
+@pytest.mark.parametrize("N,L", [(16, 2), (16, 5), (32, 3), (64, 2)])
+def test_nested_random_levels(N, L):
+    rng = np.random.default_rng(100 * N + L)
+    rho = rng.random((L, N, N, N)) * (8.0 ** np.arange(L))[:, None, None, None]
+    got, plan = _solve_gpu(rho, 2.0 / N)
+    ref = oracle.solve(rho, 2.0 / N, method="fft")
+    _assert_parity(got, ref)
+    plan.close()
+
+
+# ---------------------------------------------------------------- the five configs
+def test_config1_full_direct_sum():
+    rho = workloads.make_rho(1)
+    got, plan = _solve_gpu(rho, 2.0 / 16)
+    ref = oracle.solve(rho, 2.0 / 16, method="direct")
+    _assert_parity(got, ref)
+    plan.close()
+
+
+def test_config2_full_direct_sum():
+    rho = workloads.make_rho(2)
+    got, plan = _solve_gpu(rho, 2.0 / 32)
+    ref = oracle.solve(rho, 2.0 / 32, method="direct")
+    _assert_parity(got, ref)
+    plan.close()
+
+
+def test_config3_full_fft_oracle():
+    rho = workloads.make_rho(3)
+    got, plan = _solve_gpu(rho, 2.0 / 64)
+    ref = oracle.solve(rho, 2.0 / 64, method="fft")
+    _assert_parity(got, ref)
+    plan.close()
+
+
+def test_config4_full_fft_oracle():
+    rho = workloads.make_rho(4)
+    got, plan = _solve_gpu(rho, 2.0 / 128)
+    ref = oracle.solve(rho, 2.0 / 128, method="fft")
+    _assert_parity(got, ref)
+    plan.close()
+
+
+def test_config5_full_size_sampled_outputs_and_invariants():
+    """10 x 256^3, the configuration bench.py times (same plan, same graph launch).  The
+    oracle evaluates sampled outputs one by one by direct summation (solve_points);
+    linearity and mirror symmetry hold at any size."""
+    N, L = 256, 10
+    rho = workloads.make_rho(5)
+    got, plan = _solve_gpu(rho, 2.0 / N)
+    assert np.isfinite(got).all() and got.max() < 0
+    rng = np.random.default_rng(55)
+    targets = [(0, 0, 0, 0), (0, 128, 127, 64), (1, 255, 0, 13), (L - 1, 128, 128, 128), (L - 1, 0, 255, 77),
+               (5, 63, 64, 191), (3, 200, 31, 5)]
+    targets += [(int(rng.integers(0, 4)), *(int(v) for v in rng.integers(0, N, 3))) for _ in range(3)]
+    ref = oracle.solve_points(rho, 2.0 / N, targets)
+    for t, r in zip(targets, ref):
+        scale = np.abs(got[t[0]]).max()
+        assert abs(got[t] - r) <= TOL * scale, (t, got[t], r)
+    # mirror symmetry in x (SURVEY §8c invariants): flip input -> flipped output
+    d = torch.from_numpy(np.ascontiguousarray(rho[:, :, :, ::-1])).cuda()
+    gm = plan.potential(d).cpu().numpy()[:, :, :, ::-1]
+    for l in range(L):
+        assert np.abs(gm[l] - got[l]).max() <= TOL * np.abs(got[l]).max()
+    plan.close()
+
+
+# ---------------------------------------------------------------- edge cases and API behaviour
+def test_zero_density_gives_zero_potential():
+    rho = np.zeros((3, 16, 16, 16))
+    got, plan = _solve_gpu(rho, 0.1)
+    assert np.abs(got).max() == 0.0
+    plan.close()
+
+
+def test_coarse_density_under_fine_grid_is_ignored():
+    """Reading 10: the caller's coarse rho inside the cavity is replaced by the projection."""
+    rng = np.random.default_rng(8)
+    N, L = 16, 3
+    rho = rng.random((L, N, N, N))
+    a, plan = _solve_gpu(rho, 0.1)
+    plan.close()
+    rho2 = rho.copy()
+    lo, hi = N // 4, 3 * N // 4
+    rho2[:-1, lo:hi, lo:hi, lo:hi] = 1e9
+    b, plan = _solve_gpu(rho2, 0.1)
+    plan.close()
+    assert np.array_equal(a, b)
+
+
+def test_repeat_solves_are_bit_identical_and_graph_cache_handles_new_buffers():
+    pkg = _pkg()
+    N, L = 32, 3
+    rng = np.random.default_rng(9)
+    plan = pkg.Plan(N, L, 2.0 / N)
+    r1 = torch.from_numpy(rng.random((L, N, N, N))).cuda()
+    r2 = torch.from_numpy(rng.random((L, N, N, N))).cuda()
+    p1 = plan.potential(r1).clone()
+    p2 = plan.potential(r2).clone()
+    p1b = plan.potential(r1, torch.empty_like(r1))
+    torch.cuda.synchronize()
+    assert torch.equal(p1, p1b)
+    assert not torch.equal(p1, p2)
+    ref2 = oracle.solve(r2.cpu().numpy(), 2.0 / N)
+    _assert_parity(p2.cpu().numpy(), ref2)
+    # a side stream works too
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        p1c = plan.potential(r1, torch.empty_like(r1))
+    s.synchronize()
+    assert torch.equal(p1, p1c)
+    plan.close()
+
+
+def test_host_buffer_entry_point_matches_device_entry_point():
+    pkg = _pkg()
+    N, L = 32, 2
+    rng = np.random.default_rng(10)
+    rho = torch.from_numpy(rng.random((L, N, N, N))).pin_memory()
+    plan = pkg.Plan(N, L, 2.0 / N)
+    ph = plan.potential_host(rho)
+    pd = plan.potential(rho.cuda())
+    torch.cuda.synchronize()
+    assert torch.equal(ph, pd.cpu())
+    plan.close()
+
+
+def test_G_scales_linearly_and_error_codes():
+    pkg = _pkg()
+    rng = np.random.default_rng(11)
+    rho = rng.random((2, 16, 16, 16))
+    a, p1 = _solve_gpu(rho, 0.1, G=1.0)
+    b, p2 = _solve_gpu(rho, 0.1, G=6.674e-8)
+    assert np.abs(b - 6.674e-8 * a).max() <= 1e-15 * np.abs(b).max()
+    p1.close()
+    p2.close()
+    for bad in [dict(N=24, levels=2, dx0=1.0), dict(N=8, levels=2, dx0=1.0), dict(N=512, levels=2, dx0=1.0),
+                dict(N=16, levels=0, dx0=1.0), dict(N=16, levels=2, dx0=0.0), dict(N=16, levels=2, dx0=1.0, refinement=3)]:
+        with pytest.raises(pkg.CMError) as ei:
+            pkg.cm_plan_create(**bad)
+        assert ei.value.code == pkg.CM_EINVAL
+    h = pkg.cm_plan_create(16, 2, 0.1)
+    t = torch.zeros((2, 16, 16, 16), dtype=torch.float64, device="cuda")
+    with pytest.raises(pkg.CMError) as ei:
+        pkg.cm_potential(h, t.data_ptr(), torch.empty_like(t).data_ptr(), 0)
+    assert ei.value.code == pkg.CM_ENOTREADY
+    pkg.cm_green_precompute(h)
+    with pytest.raises(pkg.CMError) as ei:
+        pkg.cm_potential(h, t.data_ptr(), t.data_ptr(), 0)          # aliasing
+    assert ei.value.code == pkg.CM_EINVAL
+    with pytest.raises(pkg.CMError) as ei:
+        pkg.cm_potential(h, t.data_ptr() + 8, torch.empty_like(t).data_ptr(), 0)   # misaligned
+    assert ei.value.code == pkg.CM_EINVAL
+    pkg.cm_plan_destroy(h)

@@ -1,0 +1,100 @@
+"""CPU-side checks of the product: the C-ABI library builds, loads and exports every
+symbol include/cm.h declares (no compute calls without a GPU), the register DFT blocks
+are right (compiled for the host), and the shared-memory exchange layouts are free of
+bank conflicts."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_builds_loads_and_exports_every_declared_symbol():
+    import paper_2301_06763_b200 as pkg
+    so = pkg.build()
+    L = ctypes.CDLL(so)
+    hdr = open(os.path.join(ROOT, "include", "cm.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(cm_[a-z_A-Z0-9]+)\s*\(", hdr)))
+    assert len(declared) >= 10
+    for name in declared:
+        assert hasattr(L, name), f"{name} declared in cm.h but not exported"
+    assert sorted(pkg.EXPORTS) == declared
+    assert pkg.lib().cm_error_string(pkg.CM_ENOTREADY).decode().startswith("cm_green_precompute")
+
+
+def test_argument_validation_needs_no_gpu():
+    import paper_2301_06763_b200 as pkg
+    for kw in [dict(N=24, levels=2, dx0=1.0), dict(N=16, levels=2, dx0=-1.0), dict(N=16, levels=2, dx0=1.0, refinement=4)]:
+        with pytest.raises(pkg.CMError) as ei:
+            pkg.cm_plan_create(**kw)
+        assert ei.value.code == pkg.CM_EINVAL
+    assert pkg.cm_slot_to_freq(16, 0) == 0 and pkg.cm_slot_to_freq(16, 16) == 1
+    for N in (16, 64, 256):
+        f = sorted(pkg.cm_slot_to_freq(N, s) for s in range(2 * N))
+        assert f == list(range(2 * N))
+
+
+def test_product_never_touches_the_oracle():
+    """The product path must not import, link or execute anything under oracle/."""
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2301_06763_b200")):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "oracle" not in txt.lower(), f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".c")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2301_06763_b200" not in txt and "libcm.so" not in txt
+
+
+def test_register_dft_blocks_on_host(tmp_path):
+    exe = tmp_path / "hfb"
+    subprocess.run(["g++", "-std=c++17", "-O1", "-o", str(exe), os.path.join(ROOT, "tests", "host_fft_blocks.cpp")],
+                   check=True)
+    r = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout
+
+
+def _conflict_degree(addrs_complex):
+    """16-byte accesses: hardware serves a warp in quarter-warps of 8 lanes; degree = max
+    number of distinct 128-byte rows hit by the same 16-byte column within a quarter."""
+    worst = 1
+    a = np.asarray(addrs_complex)
+    for q in range(0, 32, 8):
+        cols = {}
+        for x in a[q:q + 8]:
+            cols.setdefault(x % 8, set()).add(x // 8)
+        worst = max(worst, max(len(v) for v in cols.values()))
+    return worst
+
+
+@pytest.mark.parametrize("T", [2, 4, 8, 16])
+def test_exchange_layouts_are_conflict_free(T):
+    """Mirrors LayBatch / LayRow of csrc/cm_kernels.cuh (values parsed from the source)."""
+    src = open(os.path.join(ROOT, "paper_2301_06763_b200", "csrc", "cm_kernels.cuh")).read()
+    assert "static constexpr int PS = 16 * T + 1;" in src and "static constexpr int RS = T + 1;" in src
+    assert "16 * (T + 1) + (T == 4 ? 4 : (T == 2 ? 2 : 0))" in src
+    lanes = np.arange(32)
+    # batch-fastest: px = lane & 7, j = (lane >> 3) % T, g = lane // (8 T)
+    RS, PS = T, 16 * T + 1
+    px, j, g = lanes & 7, (lanes >> 3) % T, lanes // (8 * T)
+    pen = (g * 8 + px) * PS
+    for k1 in range(16):
+        assert _conflict_degree(pen + k1 * RS + j) == 1                       # stage-1 side
+    for cc in range(16 // T):
+        for jj in range(T):
+            assert _conflict_degree(pen + (cc * T + j) * RS + jj) == 1        # stage-2 side
+    # j-fastest: j = lane % T, row = lane // T
+    RS, PS = T + 1, 16 * (T + 1) + (4 if T == 4 else (2 if T == 2 else 0))
+    j, row = lanes % T, lanes // T
+    for k1 in range(16):
+        assert _conflict_degree(row * PS + k1 * RS + j) == 1
+    for cc in range(16 // T):
+        for jj in range(T):
+            assert _conflict_degree(row * PS + (cc * T + j) * RS + jj) == 1
