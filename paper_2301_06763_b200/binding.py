@@ -16,7 +16,8 @@ from . import _build
 CM_OK, CM_EINVAL, CM_ENOMEM, CM_ECUDA, CM_ENOTREADY = 0, -1, -2, -3, -4
 CM_BUF_RESTRICTED, CM_BUF_HOLE, CM_BUF_KHAT = 0, 1, 2
 
-EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potential_host", "cm_plan_destroy",
+EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potential_host", "cm_potential_profile",
+           "cm_plan_destroy",
            "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
            "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error"]
 
@@ -38,6 +39,7 @@ def lib() -> C.CDLL:
     L.cm_green_precompute.argtypes = [vp]
     L.cm_potential.argtypes = [vp, vp, vp, vp]
     L.cm_potential_host.argtypes = [vp, vp, vp, vp]
+    L.cm_potential_profile.argtypes = [vp, vp, vp, vp, C.POINTER(C.c_float), C.c_int]
     L.cm_plan_destroy.argtypes = [vp]
     L.cm_plan_set_G.argtypes = [vp, C.c_double]
     L.cm_plan_workspace_bytes.argtypes = [vp]
@@ -79,6 +81,12 @@ def cm_potential(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0) -> None
 
 def cm_potential_host(plan: int, rho_host_ptr: int, phi_host_ptr: int, stream: int = 0) -> None:
     _check(lib().cm_potential_host(plan, rho_host_ptr, phi_host_ptr, stream), plan)
+
+
+def cm_potential_profile(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0) -> list:
+    ms = (C.c_float * 7)()
+    _check(lib().cm_potential_profile(plan, rho_ptr, phi_ptr, stream, ms, 7), plan)
+    return [float(v) for v in ms]
 
 
 def cm_plan_destroy(plan: int) -> None:
@@ -145,6 +153,14 @@ class Plan:
         s = torch.cuda.current_stream().cuda_stream if stream is None else int(stream)
         cm_potential_host(self._h, rho_host.data_ptr(), phi_host.data_ptr(), s)
         return phi_host
+
+    def potential_profile(self, rho, phi, stream=None) -> dict:
+        import torch
+        self._check_tensor(rho, "cuda")
+        self._check_tensor(phi, "cuda")
+        s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
+        ms = cm_potential_profile(self._h, rho.data_ptr(), phi.data_ptr(), s)
+        return dict(zip(["restrict", "P1_x_fwd", "P2_y_fwd", "P3_z_conv", "P4_y_inv", "P5_x_inv", "prolong_sum"], ms))
 
     def debug_buffer(self, which: int):
         import torch

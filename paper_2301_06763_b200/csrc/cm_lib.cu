@@ -66,7 +66,7 @@ template <int T> int set_attrs(cm_plan *p)
 }
 
 // The five FFT passes for every level at once (steps a3-a7).
-template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s)
+template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev)
 {
     constexpr int N = 16 * T, NN = 2 * N;
     const int L = p->L;
@@ -75,20 +75,27 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     const unsigned gy = (unsigned)((size_t)L * N * NN / (8 * (16 / T)));
     const unsigned gz = (unsigned)((size_t)NN * NN / (8 * (16 / T)) * L);
     k_x_fwd<T><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
+    if (ev) cudaEventRecord(ev[2], s);
     k_y_fwd<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    if (ev) cudaEventRecord(ev[3], s);
     k_z_conv<T><<<gz, kThreads, smem_batch<T>(), s>>>(p->W2, p->Khat, p->tw, L);
+    if (ev) cudaEventRecord(ev[4], s);
     k_y_inv<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
+    if (ev) cudaEventRecord(ev[5], s);
     k_x_inv<T><<<gx, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->tw, L, -p->G * p->dx0 * p->dx0);
+    if (ev) cudaEventRecord(ev[6], s);
     p->launches += 5;
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
 
-int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s)
+// ev (optional): 8 events; ev[0] start, ev[1] after a1, ev[2..6] after P1..P5, ev[7] after a8
+int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev = nullptr)
 {
     const int N = p->N, L = p->L, H = N / 2;
     const size_t n3 = (size_t)N * N * N, h3 = (size_t)H * H * H;
     p->launches = 0;
+    if (ev) cudaEventRecord(ev[0], s);
     // a1: restriction cascade, fine -> coarse
     for (int lf = L - 1; lf >= 1; --lf) {
         const double *rc_f = (lf < L - 1) ? p->rc + h3 * lf : nullptr;
@@ -96,13 +103,14 @@ int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s)
         p->launches++;
     }
     CM_CUDA(p, cudaGetLastError());
+    if (ev) cudaEventRecord(ev[1], s);
     int rcode = CM_EINVAL;
     switch (p->T) {
-        case 1: rcode = launch_passes<1>(p, rho, phi, s); break;
-        case 2: rcode = launch_passes<2>(p, rho, phi, s); break;
-        case 4: rcode = launch_passes<4>(p, rho, phi, s); break;
-        case 8: rcode = launch_passes<8>(p, rho, phi, s); break;
-        case 16: rcode = launch_passes<16>(p, rho, phi, s); break;
+        case 1: rcode = launch_passes<1>(p, rho, phi, s, ev); break;
+        case 2: rcode = launch_passes<2>(p, rho, phi, s, ev); break;
+        case 4: rcode = launch_passes<4>(p, rho, phi, s, ev); break;
+        case 8: rcode = launch_passes<8>(p, rho, phi, s, ev); break;
+        case 16: rcode = launch_passes<16>(p, rho, phi, s, ev); break;
     }
     if (rcode != CM_OK) return rcode;
     // a8: prolongation + Eq. 14 sum, coarse -> fine
@@ -112,6 +120,7 @@ int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s)
         p->launches++;
     }
     CM_CUDA(p, cudaGetLastError());
+    if (ev) cudaEventRecord(ev[7], s);
     return CM_OK;
 }
 
@@ -270,6 +279,22 @@ int cm_potential(cm_plan *p, const double *rho, double *phi, void *stream)
     p->graphs.push_back(ge);
     CM_CUDA(p, cudaGraphLaunch(ge.exec, s));
     return CM_OK;
+}
+
+int cm_potential_profile(cm_plan *p, const double *rho, double *phi, void *stream, float *ms_host, int n_ms)
+{
+    if (!p || !rho || !phi || !ms_host || n_ms != 7) return CM_EINVAL;
+    if (!p->green_ready) return CM_ENOTREADY;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaEvent_t ev[8];
+    for (int i = 0; i < 8; ++i) CM_CUDA(p, cudaEventCreate(&ev[i]));
+    int rc = enqueue_solve(p, rho, phi, s, ev);
+    if (rc == CM_OK && cuda_fail(p, cudaStreamSynchronize(s), "cudaStreamSynchronize")) rc = CM_ECUDA;
+    if (rc == CM_OK)
+        for (int i = 0; i < 7; ++i)
+            if (cuda_fail(p, cudaEventElapsedTime(&ms_host[i], ev[i], ev[i + 1]), "cudaEventElapsedTime")) rc = CM_ECUDA;
+    for (int i = 0; i < 8; ++i) cudaEventDestroy(ev[i]);
+    return rc;
 }
 
 int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void *stream)
