@@ -1,0 +1,402 @@
+#!/usr/bin/env python
+"""bench.py — nested-grid potential solves on B200 (and the oracle timed beside them).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is ONE whole hot path (steps a1-a8 of DESIGN.md: restriction cascade, the five
+pruned FFT passes over every level's (full, hole) pair, prolongation + Eq. 14 sum) over
+one seeded synthetic nested density field.  Default workload: BASELINE.json configs[4]
+(10 levels x 256^3, the throughput-stress config; the largest one, and it fits one GPU).
+
+Prints ONE JSON line (rank 0).  `value` = cell-updates/s (levels * N^3 * solves / s) summed
+over all ranks, inputs resident in HBM; `e2e` = the same metric through cm_potential_host
+(pinned HOST buffers, both copies inside the timed region).  Multi-GPU = replicas only
+(DESIGN.md §multi-GPU): every rank solves its own independent problem, no data-path
+collective; time = max over ranks.
+
+`--impl reference` times the ORACLE (oracle/, plain C on the host cores) on a bounded
+sample of the same workload — see run_reference().
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "nested-grid potential cell-updates/s (fp64)"
+UNIT = "cell-updates/s"
+STAGES = ["restrict", "P1_x_fwd", "P2_y_fwd", "P3_z_conv", "P4_y_inv", "P5_x_inv", "prolong_sum"]
+
+
+# --------------------------------------------------------------------------- byte models
+def algorithmic_bytes(N: int, L: int) -> dict:
+    """SURVEY.md §8(d) / DESIGN.md §5: bytes the pruned method itself must move, per LAUNCH
+    (one launch of each pass kernel processes all 2L-1 fields).  K-hat is shared by every
+    field, so it is counted once per launch."""
+    F = 2 * L - 1
+    h = (N + 1) * N * N           # half-spectrum pencils x N
+    n3 = N ** 3
+    return {
+        "P1_x_fwd": F * (8 * n3 + 16 * h),
+        "P2_y_fwd": F * (16 * h + 32 * h),
+        "P3_z_conv": F * (32 * h + 32 * h) + 8 * (N + 1) ** 3,
+        "P4_y_inv": F * (32 * h + 16 * h),
+        "P5_x_inv": F * (16 * h + 8 * n3),
+    }
+
+
+def implemented_bytes(N: int, L: int) -> dict:
+    """What the kernels as written move: one COMPLEX field per level
+    (rho_full + i rho_hole), full 2N spectrum per axis, K-hat stored as (2N)^3 reals."""
+    n3 = N ** 3
+    hole_ring = (L - 1) * (N // 2 + 2) ** 3 * 8
+    rc = (L - 1) * (N // 2) ** 3 * 8
+    return {
+        "P1_x_fwd": L * (8 * n3 + 32 * n3) + rc,
+        "P2_y_fwd": L * (32 * n3 + 64 * n3),
+        "P3_z_conv": L * (64 * n3 + 64 * n3) + 64 * n3,
+        "P4_y_inv": L * (64 * n3 + 32 * n3),
+        "P5_x_inv": L * (32 * n3 + 8 * n3) + hole_ring,
+    }
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi sampled every 100 ms while the timed region runs (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self) -> dict:
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 7:
+                    continue
+                try:
+                    sm.append(float(f[0])); smax.append(float(f[1])); pw.append(float(f[2]))
+                except ValueError:
+                    continue
+                for n, v in zip(names, f[3:7]):
+                    if v == "Active":
+                        reasons.add(n)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out.update(sm_mhz=statistics.median(sm), sm_max_mhz=max(smax), power_w_max=max(pw),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# --------------------------------------------------------------------------- distributed plumbing
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def load_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return {"hbm_gbs": float(d["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json)"}
+        except Exception:
+            pass
+    return {"hbm_gbs": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+# --------------------------------------------------------------------------- oracle timing (CPU)
+def oracle_sample(cfg_id: int, rho, steps: int, warmup: int) -> dict:
+    """Time the oracle AS IT STANDS on the host cores on a bounded sample of the workload.
+
+    One sample step = ONE field convolution (one (level, full|hole) field of the 2L-1 the
+    solve needs: oracle.field_fft, the oracle's own unpruned (2N)^3 FFT) at the workload's
+    full N, cycling through the fields; the restriction cascade and the L-1 prolongations are
+    timed once and added.  Estimated solve time = (2L-1) * mean field time + aux.
+    For N <= 32 a step is the whole solve (oracle.solve, method="fft")."""
+    import numpy as np
+    import oracle
+    import workloads
+    L, N = rho.shape[0], rho.shape[1]
+    dx0 = 2.0 / N
+    cores = oracle.num_threads()
+    if N <= 32:
+        for _ in range(warmup):
+            oracle.solve(rho, dx0, method="fft")
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            oracle.solve(rho, dx0, method="fft")
+        t_solve = (time.perf_counter() - t0) / steps
+        sample = f"{steps} whole solves (oracle.solve, method=fft) of config {cfg_id}"
+        return dict(t_solve=t_solve, cores=cores, sample=sample, steps=steps)
+    t0 = time.perf_counter()
+    rhobar = oracle.restrict(rho)
+    t_restrict = time.perf_counter() - t0
+    ghat = oracle.green_hat(N)                       # one-time, like cm_green_precompute: untimed
+    fields = [(l, h) for l in range(L) for h in ((False, True) if l < L - 1 else (False,))]
+    times = []
+    for s in range(warmup + steps):
+        l, hole = fields[s % len(fields)]
+        t0 = time.perf_counter()
+        f = oracle.field_fft(rhobar[l], hole, 1.0, dx0 / (1 << l), ghat)
+        dt = time.perf_counter() - t0
+        if s >= warmup:
+            times.append(dt)
+    t0 = time.perf_counter()
+    oracle.prolong(f)
+    t_prolong = time.perf_counter() - t0
+    t_field = sum(times) / len(times)
+    t_solve = len(fields) * t_field + t_restrict + (L - 1) * t_prolong
+    sample = (f"{steps} of the {len(fields)} field convolutions of one config-{cfg_id} solve at full N={N} "
+              f"(oracle.field_fft, mean {t_field:.3f} s each) + restriction + prolongation timed once; "
+              f"solve time = {len(fields)} x field + aux")
+    return dict(t_solve=t_solve, cores=cores, sample=sample, steps=steps, t_field=t_field)
+
+
+def run_reference(args) -> None:
+    """`--impl reference`: the oracle, unmodified, on the host cores (rank 0 only)."""
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return
+    import workloads
+    cfg = workloads.CONFIGS[args.config]
+    N, L = cfg["N"], cfg["L"]
+    rho = workloads.make_rho(args.config)
+    r = oracle_sample(args.config, rho, args.steps, args.warmup)
+    value = L * N ** 3 / r["t_solve"]
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * r["t_solve"],
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "solves_per_s": 1.0 / r["t_solve"],
+        "config": {"workload": f"config {args.config}: {cfg['name']}", "N": N, "levels": L,
+                   "note": "ms_per_step is the estimated time of one whole solve (see cpu_baseline.sample)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------- the CUDA arm
+def run_ours(args) -> None:
+    import numpy as np
+    import torch
+    import workloads
+    import paper_2301_06763_b200 as pkg
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    pkg.lib()                                        # raises if libcm.so is not built
+    cfg = workloads.CONFIGS[args.config]
+    N, L = cfg["N"], cfg["L"]
+    dx0 = 2.0 / N
+    rho_np = workloads.make_rho(args.config)
+    plan = pkg.Plan(N, L, dx0)
+    rho = torch.from_numpy(rho_np).to(dev)
+    phi = torch.empty_like(rho)
+    cells = L * N ** 3
+    launches_per_step = plan.kernel_launches
+    stream = torch.cuda.current_stream(dev)
+
+    # L2 hygiene: at N >= 128 one solve streams > 10x the 126 MB L2 through every pass, so
+    # the inputs themselves evict it; below that, write a 256 MB buffer between timed steps.
+    flush = None
+    ws = plan.workspace_bytes
+    if ws < (1 << 30):
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def step():
+        if flush is not None:
+            flush.fill_(1)
+        plan.potential(rho, phi)
+
+    # ---- region 1: K whole solves through cm_potential (CUDA-graph launch), device resident
+    for _ in range(max(args.warmup, 3)):
+        step()
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    if flush is None:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        barrier()
+        ms_total = e0.elapsed_time(e1)
+    else:                                            # time each solve, excluding the flush kernel
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in evs:
+            flush.fill_(1)
+            a.record(stream)
+            plan.potential(rho, phi)
+            b.record(stream)
+        barrier()
+        ms_total = sum(a.elapsed_time(b) for a, b in evs)
+    ms_step = max_over_ranks(ms_total / args.steps)
+
+    # ---- region 2: the same K solves launched kernel by kernel with CUDA events between the
+    # stages (cm_potential_profile) — per-kernel durations for the roofline, measured live.
+    acc = {k: 0.0 for k in STAGES}
+    for _ in range(args.steps):
+        if flush is not None:
+            flush.fill_(1)
+        for k, v in plan.potential_profile(rho, phi).items():
+            acc[k] += v
+    stage_ms = {k: v / args.steps for k, v in acc.items()}
+    clocks = sampler.stop() if rank == 0 else {}
+    barrier()
+
+    # ---- region 3: end to end through cm_potential_host (pinned host buffers, H2D + D2H timed)
+    rho_h = torch.from_numpy(rho_np).pin_memory()
+    phi_h = torch.empty_like(rho_h).pin_memory()
+    e2e_steps = max(3, min(args.steps, 10))
+    plan.potential_host(rho_h, phi_h)
+    barrier()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        plan.potential_host(rho_h, phi_h)
+    e1.record(stream)
+    barrier()
+    wall_e2e = (time.perf_counter() - t0) / e2e_steps * 1e3      # the call is synchronous: host clock counts too
+    ms_e2e = max_over_ranks(max(e0.elapsed_time(e1) / e2e_steps, wall_e2e))
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel
+    peaks = load_peaks()
+    alg, impl = algorithmic_bytes(N, L), implemented_bytes(N, L)
+    dom = max(alg.keys(), key=lambda k: stage_ms[k])
+    achieved = alg[dom] / (stage_ms[dom] * 1e-3) / 1e9
+    per_pass = {k: {"ms": round(stage_ms[k], 4),
+                    "alg_GBs": round(alg[k] / (stage_ms[k] * 1e-3) / 1e9, 1) if stage_ms[k] > 0 else None,
+                    "impl_GBs": round(impl[k] / (stage_ms[k] * 1e-3) / 1e9, 1) if stage_ms[k] > 0 else None}
+                for k in alg}
+    solve_alg_bytes = (2 * L - 1) * (16 * N ** 3 + 192 * (N + 1) * N * N) + 8 * (N + 1) ** 3
+    roofline = {
+        "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+        "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
+        "algorithmic_bytes_per_launch": alg[dom], "implemented_bytes_per_launch": impl[dom],
+        "kernel_ms": stage_ms[dom], "per_pass": per_pass,
+        "aux_ms": {"restrict": round(stage_ms["restrict"], 4), "prolong_sum": round(stage_ms["prolong_sum"], 4)},
+        "stage_sum_ms": sum(stage_ms.values()),
+        "whole_solve_alg_GBs": solve_alg_bytes / (ms_step * 1e-3) / 1e9,
+        "whole_solve_frac": solve_alg_bytes / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"],
+    }
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")   # written by hand from an ncu --set full capture
+    if os.path.exists(traffic_file):
+        try:
+            roofline["traffic"] = json.load(open(traffic_file)).get(f"config{args.config}", {}).get(dom)
+        except Exception:
+            pass
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        r = oracle_sample(args.config, rho_np, 2 if N > 32 else 3, 0)
+        cpu = {"value": cells / r["t_solve"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]}
+
+    value = world * cells / (ms_step * 1e-3)
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "solves_per_s": world / (ms_step * 1e-3),
+        "config": {"workload": f"config {args.config}: {cfg['name']}", "N": N, "levels": L, "fields": 2 * L - 1,
+                   "parallelism": "replicas only" if world > 1 else "single GPU",
+                   "l2": ("inputs larger than L2 (workspace %.1f GB streamed per solve)" % (ws / 1e9)) if flush is None
+                         else "256 MB flush buffer written between timed solves",
+                   "launch": "cm_potential -> cudaGraphLaunch of %d kernels" % launches_per_step},
+        "clocks": clocks,
+        "e2e": {"value": world * cells / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                "h2d_bytes_per_step": rho_h.numel() * 8, "d2h_bytes_per_step": phi_h.numel() * 8,
+                "api": "cm_potential_host (pinned host rho -> device -> solve -> pinned host phi)"},
+        "gpu_launches": args.steps * launches_per_step,
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    plan.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)       # the paper's protocol: 20 full cycles
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
