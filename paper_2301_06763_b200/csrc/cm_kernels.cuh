@@ -61,12 +61,30 @@ template <int T> struct LayRow {
 struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
 struct SyncWarp  { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
 
+// ---- twiddle sources ------------------------------------------------------------------
+// w_2N^{j (2 k1 + P)}: from the global table (read-only path) or from a per-CTA shared copy
+// laid out [2 k1 + P][j] so that consecutive j are consecutive 16-byte words.
+struct TwGlobal {
+    const double2 *__restrict__ tw;
+    int j;
+    template <int P> __device__ __forceinline__ double2 get(int k1) const { return __ldg(&tw[j * (2 * k1 + P)]); }
+};
+template <int T> struct TwShared {
+    const double2 *base;   // table + j
+#ifndef ABL_NOTW
+    template <int P> __device__ __forceinline__ double2 get(int k1) const { return base[(2 * k1 + P) * T]; }
+#else
+    template <int P> __device__ __forceinline__ double2 get(int k1) const { return make_double2(0.6 + k1, 0.8 - P); }
+#endif
+};
+
 // ---- half transforms ---------------------------------------------------------------
 // Forward, parity P: a[r] = input element n = j + T r (r < 16).  On return
 // v[cc*T + k2] is the spectrum value of slot  P*N + 16*k2 + cc*T + j.
-template <int T, int P, class Lay, class Sync>
-__device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16], int j, double2 *sm,
-                                         const double2 *__restrict__ tw, Sync sync)
+// PRE: synchronise before writing the exchange buffer (needed when one buffer serves
+// consecutive exchanges).
+template <int T, int P, class Lay, bool PRE = false, class Sync, class Tw>
+__device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16], int j, double2 *sm, Tw tw, Sync sync)
 {
     double2 b[16];
 #pragma unroll
@@ -74,16 +92,26 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
     if (P) ModW32<15, -1>::run(b);
     Dft<16, -1>::run(b);
     if (T > 1) {
+        if (PRE) sync();
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
-            if (k1 > 0 || P) b[k1] = cmul(b[k1], __ldg(&tw[j * (2 * k1 + P)]));
+            if (k1 > 0 || P) b[k1] = cmul(b[k1], tw.template get<P>(k1));
+#ifndef ABL_NOEX
             sm[k1 * Lay::RS + j] = b[k1];
+#endif
         }
+#ifndef ABL_NOEX
         sync();
+#endif
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc) {
+#ifndef ABL_NOEX
 #pragma unroll
             for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = sm[(cc * T + j) * Lay::RS + jj];
+#else
+#pragma unroll
+            for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = b[cc * T + jj];
+#endif
             Dft<T, -1>::run(&v[cc * T]);
         }
     } else {
@@ -95,22 +123,30 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
 // Inverse, parity P: v as above (consumed); on return o[r] is parity P's contribution
 // to output element n = j + T r, r < 16 (the cropped half), already multiplied by
 // conj(w_32^r) for P = 1.
-template <int T, int P, class Lay, class Sync>
-__device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm,
-                                         const double2 *__restrict__ tw, Sync sync)
+template <int T, int P, class Lay, bool PRE = false, class Sync, class Tw>
+__device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm, Tw tw, Sync sync)
 {
     if (T > 1) {
+        if (PRE) sync();
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc) {
             Dft<T, +1>::run(&v[cc * T]);
+#ifndef ABL_NOEX
 #pragma unroll
             for (int jj = 0; jj < T; ++jj) sm[(cc * T + j) * Lay::RS + jj] = v[cc * T + jj];
+#endif
         }
+#ifndef ABL_NOEX
         sync();
+#endif
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
+#ifndef ABL_NOEX
             o[k1] = sm[k1 * Lay::RS + j];
-            if (k1 > 0 || P) o[k1] = cmulc(o[k1], __ldg(&tw[j * (2 * k1 + P)]));
+#else
+            o[k1] = v[k1];
+#endif
+            if (k1 > 0 || P) o[k1] = cmulc(o[k1], tw.template get<P>(k1));
         }
     } else {
 #pragma unroll
@@ -153,7 +189,7 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ r
     double2 *dst = W1 + row * NN;
     {
         double2 v[16];
-        fwd_half<T, 0, Lay>(a, v, j, bufA, tw, SyncWarp());
+        fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncWarp());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
@@ -161,7 +197,7 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ r
     }
     {
         double2 v[16];
-        fwd_half<T, 1, Lay>(a, v, j, bufB, tw, SyncWarp());
+        fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, SyncWarp());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
@@ -193,8 +229,8 @@ __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ 
             v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
         }
     double2 e[16], o[16];
-    inv_half<T, 0, Lay>(v0, e, j, bufA, tw, SyncWarp());
-    inv_half<T, 1, Lay>(v1, o, j, bufB, tw, SyncWarp());
+    inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
+    inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncWarp());
 
     const double scale = scale0 * exp2(-2.0 * b);   // dx_b^2 = dx0^2 / 4^b, exact
     const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
@@ -232,7 +268,7 @@ __global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ 
     for (int r = 0; r < 16; ++r) a[r] = src[(size_t)(j + T * r) * NN];
     {
         double2 v[16];
-        fwd_half<T, 0, Lay>(a, v, j, bufA, tw, SyncBlock());
+        fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncBlock());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
@@ -240,7 +276,7 @@ __global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ 
     }
     {
         double2 v[16];
-        fwd_half<T, 1, Lay>(a, v, j, bufB, tw, SyncBlock());
+        fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, SyncBlock());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
@@ -273,8 +309,8 @@ __global__ void __launch_bounds__(kThreads) k_y_inv(const double2 *__restrict__ 
             v1[cc * T + k2] = src[(size_t)(N + 16 * k2 + cc * T + j) * NN];
         }
     double2 e[16], o[16];
-    inv_half<T, 0, Lay>(v0, e, j, bufA, tw, SyncBlock());
-    inv_half<T, 1, Lay>(v1, o, j, bufB, tw, SyncBlock());
+    inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncBlock());
+    inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncBlock());
 #pragma unroll
     for (int r = 0; r < 16; ++r) dst[(size_t)(j + T * r) * NN] = cadd(e[r], o[r]);
 }
@@ -304,7 +340,7 @@ __global__ void __launch_bounds__(kThreads) k_z_conv(double2 *__restrict__ W2, c
     double2 e[16];
     {
         double2 v[16];
-        fwd_half<T, 0, Lay>(a, v, j, bufA, tw, SyncBlock());
+        fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncBlock());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
@@ -313,11 +349,11 @@ __global__ void __launch_bounds__(kThreads) k_z_conv(double2 *__restrict__ W2, c
                 v[cc * T + k2].x *= k;
                 v[cc * T + k2].y *= k;
             }
-        inv_half<T, 0, Lay>(v, e, j, bufB, tw, SyncBlock());
+        inv_half<T, 0, Lay>(v, e, j, bufB, TwGlobal{tw, j}, SyncBlock());
     }
     {
         double2 v[16], o[16];
-        fwd_half<T, 1, Lay>(a, v, j, bufA, tw, SyncBlock());
+        fwd_half<T, 1, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncBlock());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
@@ -326,7 +362,7 @@ __global__ void __launch_bounds__(kThreads) k_z_conv(double2 *__restrict__ W2, c
                 v[cc * T + k2].x *= k;
                 v[cc * T + k2].y *= k;
             }
-        inv_half<T, 1, Lay>(v, o, j, bufB, tw, SyncBlock());
+        inv_half<T, 1, Lay>(v, o, j, bufB, TwGlobal{tw, j}, SyncBlock());
 #pragma unroll
         for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
     }

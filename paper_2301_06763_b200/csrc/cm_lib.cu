@@ -10,6 +10,7 @@
 
 #include "../../include/cm.h"
 #include "cm_kernels.cuh"
+#include "cm_zconv.cuh"
 
 namespace {
 
@@ -34,6 +35,11 @@ struct cm_plan {
     cudaStream_t cap_stream = nullptr;
     std::vector<GraphEntry> graphs;
     int launches = 0;
+    int num_sms = 148;
+    int zconv_grid = 0;
+    int zconv_mode = 0;             // 2 = parity-split direct kernel
+    bool zconv_tma = true;          // P3 through the TMA-fed persistent kernel (CM_ZCONV=direct selects the first version)
+    CUtensorMap mapW, mapK;
     char err[512] = {0};
 };
 
@@ -62,6 +68,9 @@ template <int T> int set_attrs(cm_plan *p)
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_ps<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T))));
+    CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
     return CM_OK;
 }
 
@@ -78,7 +87,20 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     if (ev) cudaEventRecord(ev[2], s);
     k_y_fwd<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     if (ev) cudaEventRecord(ev[3], s);
-    k_z_conv<T><<<gz, kThreads, smem_batch<T>(), s>>>(p->W2, p->Khat, p->tw, L);
+    if (p->zconv_mode == 2) {
+        const size_t sm = sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T);
+        const int ntile = NN * NN / (8 * (16 / T));
+        int lo = p->zconv_grid > 0 ? p->zconv_grid : 64;
+        while (ntile % lo) lo >>= 1;
+        k_z_conv_ps<T><<<gz, 256, sm, s>>>(p->W2, p->Khat, p->tw, L, lo);
+    } else if (p->zconv_tma) {
+        const int ngroups = NN * NN / ZConvCfg<T>::PEN;
+        int grid = ngroups < 2 * p->num_sms ? ngroups : 2 * p->num_sms;
+        if (p->zconv_grid > 0 && p->zconv_grid < grid) grid = p->zconv_grid;
+        k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->mapK, p->W2, p->tw, L, ngroups);
+    } else {
+        k_z_conv<T><<<gz, kThreads, smem_batch<T>(), s>>>(p->W2, p->Khat, p->tw, L);
+    }
     if (ev) cudaEventRecord(ev[4], s);
     k_y_inv<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
     if (ev) cudaEventRecord(ev[5], s);
@@ -148,6 +170,51 @@ template <class Tp> int dev_alloc(cm_plan *p, Tp **ptr, size_t count)
     return CM_OK;
 }
 
+// TMA descriptors for P3 (cm_zconv.cuh).  cuTensorMapEncodeTiled is a driver entry point;
+// it is looked up through the runtime so that libcm does not link libcuda directly.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int make_tensor_maps(cm_plan *p)
+{
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    CM_CUDA(p, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+    if (!fn || q != cudaDriverEntryPointSuccess) {
+        std::snprintf(p->err, sizeof(p->err), "cuTensorMapEncodeTiled not available from this driver");
+        return CM_ECUDA;
+    }
+    EncodeTiledFn enc = (EncodeTiledFn)fn;
+    const cuuint64_t NN = 2 * (cuuint64_t)p->N, N = p->N, L = p->L;
+    const cuuint32_t es[2] = {1, 1};
+    {   // W2 as fp64 [L*N rows][2*(2N)^2]; box = 16 doubles (8 complex = 128 B) x N rows, 128B swizzle
+        const cuuint64_t dims[2] = {2 * NN * NN, L * N};
+        const cuuint64_t strides[1] = {NN * NN * 16};
+        const cuuint32_t box[2] = {16, (cuuint32_t)N};
+        CUresult r = enc(&p->mapW, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->W2, dims, strides, box, es,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            std::snprintf(p->err, sizeof(p->err), "cuTensorMapEncodeTiled(W2) failed: %d", (int)r);
+            return CM_ECUDA;
+        }
+    }
+    {   // K-hat as fp64 [2N rows][(2N)^2]; box = 8 doubles (64 B) x min(2N, 256) rows, 64B swizzle
+        const cuuint64_t dims[2] = {NN * NN, NN};
+        const cuuint64_t strides[1] = {NN * NN * 8};
+        const cuuint32_t box[2] = {8, (cuuint32_t)(NN < 256 ? NN : 256)};
+        CUresult r = enc(&p->mapK, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->Khat, dims, strides, box, es,
+                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            std::snprintf(p->err, sizeof(p->err), "cuTensorMapEncodeTiled(K-hat) failed: %d", (int)r);
+            return CM_ECUDA;
+        }
+    }
+    return CM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -200,6 +267,18 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         else if (cuda_fail(p, cudaMemset(p->hole, 0, L * n3 * sizeof(double)), "cudaMemset")) rc = CM_ECUDA;
         else if (cuda_fail(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking), "cudaStreamCreate"))
             rc = CM_ECUDA;
+    }
+    if (rc == CM_OK) {
+        const char *zc = std::getenv("CM_ZCONV");
+        p->zconv_tma = !(zc && std::strcmp(zc, "direct") == 0);
+        if (zc && std::strcmp(zc, "ps") == 0) p->zconv_mode = 2;
+        const char *zg = std::getenv("CM_ZCONV_GRID");
+        p->zconv_grid = zg ? std::atoi(zg) : 0;
+        int dev = 0;
+        if (cuda_fail(p, cudaGetDevice(&dev), "cudaGetDevice") ||
+            cuda_fail(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
+            rc = CM_ECUDA;
+        else if (p->zconv_tma) rc = make_tensor_maps(p);
     }
     if (rc == CM_OK) {
         switch (p->T) {

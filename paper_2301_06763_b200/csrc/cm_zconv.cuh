@@ -1,0 +1,345 @@
+// cm_zconv.cuh — P3 (step a5): z forward * K-hat * z inverse, TMA-fed persistent kernel.
+//
+// PAPER.md:L118-L123 (Eq. 11): the convolution is a product in Fourier space.  The z axis
+// is the last one transformed, so the forward z transform, the multiplication by the real
+// K-hat and the inverse z transform of one pencil happen in registers without the
+// (2N)^3 spectrum ever reaching memory.
+//
+// Why this shape (profiles/r01a_ncu_full_config5.md): the first k_z_conv was neither
+// DRAM- nor fp64-bound; its 8 warps/SM stalled on the tile load, on K-hat loads issued in
+// the middle of the dependency chain and on CTA-wide barriers.  Here
+//   * a CTA is persistent and walks tiles (g, b): g = a group of PEN adjacent (sy,sx)
+//     pencils, b = level.  All L levels of a group run back to back so the group's
+//     K-hat tile is fetched ONCE (TMA, 64B-swizzled) and stays in shared memory;
+//   * the next tile's W2 data ([N z-rows][128 B], stride (2N)^2) is fetched by TMA
+//     (128B-swizzled box) while the current tile is being transformed; the tile is copied
+//     to registers as soon as it lands, which frees the stage for the following load;
+//   * the T threads that share a pencil sit in ONE warp (j fastest), so the radix-16 x
+//     radix-T exchange needs __syncwarp only; twiddles come from a shared-memory copy.
+// Output is staged in shared memory (the idle exchange buffer) and written by a TMA store:
+// writing it straight from registers (32-byte sectors per row per warp with this thread
+// mapping) cost 6 ms of the 10.6 ms at N = 256 (ablation).
+#pragma once
+
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "cm_kernels.cuh"
+
+namespace cmk {
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap *map, int c0, int c1, uint32_t bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(c0), "r"(c1)
+        : "memory");
+}
+
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap *map, int c0, int c1, uint32_t src)
+{
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];" ::"l"(map), "r"(src), "r"(c0),
+                 "r"(c1)
+                 : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+
+template <int T> struct ZConvCfg {
+    static constexpr int N = 16 * T, NN = 2 * N;
+    static constexpr int PEN = kThreads / T;          // pencils per tile
+    static constexpr int NBOX = PEN / 8;              // 128-byte column groups per tile
+    static constexpr int PPW = 32 / T;                // pencils per warp
+    static constexpr int KROWS = NN < 256 ? NN : 256; // rows of one K-hat TMA box (box dims <= 256)
+    static constexpr int KCH = NN / KROWS;
+    static constexpr uint32_t IN_BYTES = 32768, KH_BYTES = 32768;
+    // exchange buffer; at the end of a tile the same bytes stage the output tile for the TMA store
+    static constexpr uint32_t EX_BYTES = (T > 1) ? PEN * LayRow<T>::PS * 16 : 32768;
+    static_assert(EX_BYTES >= 32768, "the exchange buffer doubles as the 32 KB output stage");
+    static constexpr uint32_t TW_BYTES = 32 * T * 16;
+    static constexpr uint32_t OFF_IN = 0, OFF_KH = IN_BYTES, OFF_EX = OFF_KH + KH_BYTES, OFF_TW = OFF_EX + EX_BYTES,
+                              OFF_BAR = OFF_TW + TW_BYTES;
+    static constexpr uint32_t SMEM = OFF_BAR + 16 + 1024;   // + slack for the manual 1024-byte alignment
+};
+
+template <int T>
+__global__ void __launch_bounds__(kThreads, 2)
+k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapK,
+             double2 *__restrict__ W2, const double2 *__restrict__ tw, int L, int ngroups)
+{
+    using C = ZConvCfg<T>;
+    constexpr int N = C::N, NN = C::NN, PEN = C::PEN, NBOX = C::NBOX;
+    using Lay = LayRow<T>;
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t s0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char *sbase = smem_raw + (s0 - smem_u32(smem_raw));
+    const uint32_t bar_in = s0 + C::OFF_BAR, bar_k = bar_in + 8;
+    double2 *ex_s = reinterpret_cast<double2 *>(sbase + C::OFF_EX);
+    double2 *tw_s = reinterpret_cast<double2 *>(sbase + C::OFF_TW);
+
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31, j = lane % T, pxl = lane / T;
+    const int pen = w * C::PPW + pxl, bx = pen >> 3, px = pen & 7;
+    const size_t zs = (size_t)NN * NN;
+
+    if ((int)blockIdx.x >= ngroups) return;
+    const int my_groups = (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int ntiles = my_groups * L;
+
+    auto issue_in = [&](int g, int b) {
+        // the stage was last touched through the generic proxy (LDS): order those accesses before
+        // the async-proxy write.  Without this fence the refill raced with them (measured: wrong
+        // results whenever two CTAs shared an SM).
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(bar_in, C::IN_BYTES);
+#pragma unroll
+        for (int q = 0; q < NBOX; ++q)
+            tma_load_2d(s0 + C::OFF_IN + q * (N * 128), &mapW, 2 * (g * PEN + 8 * q), b * N, bar_in);
+    };
+    auto issue_k = [&](int g) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(bar_k, C::KH_BYTES);
+#pragma unroll
+        for (int q = 0; q < NBOX; ++q)
+#pragma unroll
+            for (int c = 0; c < C::KCH; ++c)
+                tma_load_2d(s0 + C::OFF_KH + q * (NN * 64) + c * (C::KROWS * 64), &mapK, g * PEN + 8 * q, c * C::KROWS, bar_k);
+    };
+
+    if (tid == 0) {
+        mbar_init(bar_in, 1);
+        mbar_init(bar_k, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = tid; i < 32 * T; i += kThreads) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
+    __syncthreads();
+    if (tid == 0) {
+        issue_k((int)blockIdx.x);
+        issue_in((int)blockIdx.x, 0);
+    }
+
+    const unsigned char *in_p = sbase + C::OFF_IN + bx * (N * 128);
+    const unsigned char *kh_p = sbase + C::OFF_KH + bx * (NN * 64) + ((px & 1) << 3);
+    double2 *ex_p = ex_s + pen * Lay::PS;
+#ifdef ZC_TWGLOBAL
+    const TwGlobal tws{tw, j};
+#else
+    const TwShared<T> tws{tw_s + j};
+#endif
+#ifdef ZC_SYNCBLOCK
+    using SyncX = SyncBlock;
+#else
+    using SyncX = SyncWarp;
+#endif
+    uint32_t ph_in = 0, ph_k = 0;
+
+    for (int t = 0; t < ntiles; ++t) {
+        const int gi = t / L, b = t - gi * L;
+        const int g = (int)blockIdx.x + gi * (int)gridDim.x;
+
+        mbar_wait(bar_in, ph_in);
+        ph_in ^= 1;
+        double2 a[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int z = j + T * r;
+            a[r] = *reinterpret_cast<const double2 *>(in_p + z * 128 + ((px ^ (z & 7)) << 4));
+        }
+        if (tid == 0) tma_store_wait_read();   // the previous tile's output has left the exchange/out buffer
+        __syncthreads();   // every thread holds its part of the tile: the stage may be refilled
+        if (tid == 0 && t + 1 < ntiles) {
+            if (b + 1 < L) issue_in(g, b + 1);
+            else issue_in(g + (int)gridDim.x, 0);
+        }
+
+        auto kmul = [&](double2(&v)[16], int P) {
+#pragma unroll
+            for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+                for (int k2 = 0; k2 < T; ++k2) {
+                    const int s = P * N + 16 * k2 + cc * T + j;
+                    const double k = *reinterpret_cast<const double *>(kh_p + s * 64 + ((((px >> 1) ^ (s >> 1)) & 3) << 4));
+                    v[cc * T + k2].x *= k;
+                    v[cc * T + k2].y *= k;
+                }
+        };
+
+#ifdef ZC_NOCOMPUTE
+        double2 e[16];
+        if (b == 0) { mbar_wait(bar_k, ph_k); ph_k ^= 1; }
+#pragma unroll
+        for (int r = 0; r < 16; ++r) e[r] = a[r];
+        kmul(e, 0);
+        if (b == L - 1 && t + 1 < ntiles) { __syncthreads(); if (tid == 0) issue_k(g + (int)gridDim.x); }
+#else
+        double2 e[16];
+        {
+            double2 v[16];
+            fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncX());
+            if (b == 0) {
+                mbar_wait(bar_k, ph_k);
+                ph_k ^= 1;
+            }
+            kmul(v, 0);
+            inv_half<T, 0, Lay, true>(v, e, j, ex_p, tws, SyncX());
+        }
+        {
+            double2 v[16], o[16];
+            fwd_half<T, 1, Lay, true>(a, v, j, ex_p, tws, SyncX());
+            kmul(v, 1);
+            if (b == L - 1 && t + 1 < ntiles) {   // last use of this group's K-hat tile
+                __syncthreads();
+                if (tid == 0) issue_k(g + (int)gridDim.x);
+            }
+            inv_half<T, 1, Lay, true>(v, o, j, ex_p, tws, SyncX());
+#pragma unroll
+            for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
+        }
+#endif
+        // stage the output tile in the (now idle) exchange buffer with the box layout of the
+        // input stage, then one thread hands it to the TMA unit: full 128-byte rows to L2.
+        __syncthreads();   // every warp is done with its exchanges
+        {
+            unsigned char *out_p = sbase + C::OFF_EX + bx * (N * 128);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const int z = j + T * r;
+#ifdef ZC_NOSTORE
+                if (e[r].x == 1.2345e-300)
+#endif
+                *reinterpret_cast<double2 *>(out_p + z * 128 + ((px ^ (z & 7)) << 4)) = e[r];
+            }
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+#ifndef ZC_NOSTORE
+#pragma unroll
+            for (int q = 0; q < NBOX; ++q)
+                tma_store_2d(&mapW, 2 * (g * PEN + 8 * q), b * N, s0 + C::OFF_EX + q * (N * 128));
+            tma_store_commit();
+#endif
+        }
+    }
+    if (tid == 0) tma_store_wait_all();
+}
+
+
+// ====================== P3, parity-split variant (no TMA) ==========================
+// 256 threads: warps 0-3 take the even output frequencies (P = 0), warps 4-7 the odd ones
+// (P = 1) of the SAME 8*G pencils.  Each thread carries one parity only, which halves the
+// live registers (<= 128 -> 16 warps per SM instead of 8) and the serial work per thread;
+// the two partial inverse transforms are summed through shared memory at the end.
+struct NamedBar {
+    int id;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+};
+
+template <int T, int P>
+__device__ __forceinline__ void zconv_ps_half(const double2 (&a)[16], const double (&kk)[16], double2 (&o)[16], int j,
+                                              double2 *buf, const TwShared<T> &tws)
+{
+    using Lay = LayBatch<T>;
+    double2 v[16];
+    fwd_half<T, P, Lay, false>(a, v, j, buf, tws, NamedBar{1 + P});
+#pragma unroll
+    for (int i = 0; i < 16; ++i) {
+        v[i].x *= kk[i];
+        v[i].y *= kk[i];
+    }
+    inv_half<T, P, Lay, true>(v, o, j, buf, tws, NamedBar{1 + P});
+}
+
+template <int T>
+__global__ void __launch_bounds__(256, 2) k_z_conv_ps(double2 *__restrict__ W2, const double *__restrict__ Khat,
+                                                      const double2 *__restrict__ tw, int L, int lo_tiles)
+{
+    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    using Lay = LayBatch<T>;
+    extern __shared__ double2 smem[];
+    double2 *tw_s = smem + 2 * PEN * Lay::PS;
+    const int P = threadIdx.x >> 7, t = threadIdx.x & 127, px = t & 7, j = (t >> 3) % T, g = t / (8 * T);
+    // block order: [tile_hi][b][tile_lo], tile_lo < lo_tiles: lo_tiles adjacent tiles of one level run
+    // together (contiguous lo_tiles*PEN*16 bytes per z row -> DRAM page locality), and their K-hat
+    // tiles (lo_tiles * 32 KB) stay in L2 across the L levels.
+    const int chunk = lo_tiles * L;
+    const int hi = blockIdx.x / chunk, rem = blockIdx.x - hi * chunk;
+    const int b = rem / lo_tiles, tile = hi * lo_tiles + (rem - b * lo_tiles);
+    const size_t flat = (size_t)tile * PEN + g * 8 + px;   // sy * 2N + sx
+    const size_t zs = (size_t)NN * NN;
+    double2 *base = W2 + (size_t)b * N * zs + flat;
+    const double *kh = Khat + flat + (size_t)P * N * zs;
+    double2 *buf = smem + (P * PEN + g * 8 + px) * Lay::PS;
+    double2 *buf1 = smem + (PEN + g * 8 + px) * Lay::PS;               // the odd group's buffer
+
+    double2 a[16];
+    double kk[16];
+#ifndef ABL_NOGLOBAL
+#pragma unroll
+    for (int r = 0; r < 16; ++r) a[r] = base[(size_t)(j + T * r) * zs];
+#pragma unroll
+    for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+        for (int k2 = 0; k2 < T; ++k2) kk[cc * T + k2] = __ldg(kh + (size_t)(16 * k2 + cc * T + j) * zs);
+#else
+#pragma unroll
+    for (int r = 0; r < 16; ++r) { a[r] = make_double2(threadIdx.x + r, blockIdx.x - r); kk[r] = 0.5 + r; }
+#endif
+    for (int i = threadIdx.x; i < 32 * T; i += 256) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
+    __syncthreads();
+    const TwShared<T> tws{tw_s + j};
+
+    double2 o[16];
+#ifdef ABL_NOCOMPUTE
+    if (P == 0) {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) base[(size_t)(j + T * r) * zs] = make_double2(a[r].x * kk[r], a[r].y);
+    }
+    return;
+#endif
+    if (P == 0) {
+        zconv_ps_half<T, 0>(a, kk, o, j, buf, tws);
+        __syncthreads();                       // the odd half's partial result is in buf1
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const double2 res = cadd(o[r], buf1[r * T + j]);
+#ifdef ABL_NOGLOBAL
+            if (res.x == 1.2345e-300)
+#endif
+            base[(size_t)(j + T * r) * zs] = res;
+        }
+    } else {
+        zconv_ps_half<T, 1>(a, kk, o, j, buf, tws);
+        NamedBar{2}();                         // every odd-group thread is done reading the exchange buffer
+#pragma unroll
+        for (int r = 0; r < 16; ++r) buf[r * T + j] = o[r];
+        __syncthreads();
+    }
+}
+
+}  // namespace cmk
