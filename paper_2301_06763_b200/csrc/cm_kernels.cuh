@@ -9,8 +9,8 @@
 //   P2 k_y_fwd : W1          -> W2[b][z<N][sy<2N][sx<2N]
 //   P3 k_z_conv: W2 in place    z transform, * K-hat (Eq. 11), inverse z, keep z < N
 //   P4 k_y_inv : W2          -> W1[b][z<N][y<N][sx<2N]
-//   P5 k_x_inv : W1          -> phi (Re) and hole (Im), scaled by -G dx_b^2, x < N kept
-//   phi,hole --k_prolong_sum (coarse->fine cascade, Eq. 3-6 + Eq. 14)--> phi
+//   P5 k_x_inv : W1          -> phi (Re) and hole (Im), scaled by -G dx_b^2, x < N kept; one launch per level,
+//                coarse -> fine, adding the prolonged ext_b = P[ext_{b-1} + Phi_hole^{b-1}] (Eq. 3-6 + Eq. 14, step a8)
 //
 // "sx, sy, sz" are storage slots, not frequencies: slot s = p N + 16 k2 + k1 holds
 // frequency 2 k1 + p + 32 k2 (cm_fft.cuh).  The order is whatever makes every global
@@ -164,13 +164,15 @@ __device__ __forceinline__ bool in_ring1(int v, int N) { return v >= N / 4 - 1 &
 // pair field (step a2, never materialised), writes 2N complex slots.
 template <int T>
 __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ rho, const double *__restrict__ rc,
-                                                    double2 *__restrict__ W1, const double2 *__restrict__ tw, int L)
+                                                    double2 *__restrict__ W1, const double2 *__restrict__ tw, int L,
+                                                    size_t row0)
 {
+    // row0: first global row (b, z, y) of this launch
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, H = N / 2, Q = N / 4;
     using Lay = LayRow<T>;
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
-    const size_t row = (size_t)blockIdx.x * ROWS + rowl;
+    const size_t rowc = (size_t)blockIdx.x * ROWS + rowl, row = row0 + rowc;
     const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
     const bool finest = (b == L - 1);
     const bool rowcav = !finest && in_cavity1(z, N) && in_cavity1(y, N);
@@ -205,17 +207,26 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ r
     }
 }
 
-// ================================ P5: x inverse ====================================
+// ====================== P5: x inverse + a8 (prolongation, Eq. 14) ==================
+// One launch per level b, coarse -> fine (row0 = b N^2): the level's rows are transformed back,
+// cropped to x < N and scaled by -G dx_b^2; then the contribution of the coarser levels is added
+// on the spot (step a8): with Hc = ext_{b-1} + Phi_hole^{b-1} on the parent grid (valid on the
+// cavity grown by one cell, written by the previous launch), a fine cell f with parent
+// p = N/4 + f/2 and sign s = +1 (f odd) / -1 (f even) gets
+//     ext_b(f) = 3/4 Hc[p] + 1/4 Hc[p+s]        (Eq. 3-6)
+//     Phi(Omega_b) = Phi^b + ext_b               (Eq. 14)
+// and hole_b = Phi_hole^b + ext_b is kept where the next level will read it.
 template <int T>
 __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
-                                                    double *__restrict__ hole, const double2 *__restrict__ tw,
-                                                    int L, double scale0 /* -G dx0^2 */)
+                                                    double *__restrict__ hole, const double *__restrict__ hole_c,
+                                                    const double2 *__restrict__ tw, int L, double scale0 /* -G dx0^2 */,
+                                                    size_t row0)
 {
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T;
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, Q = N / 4;
     using Lay = LayRow<T>;
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
-    const size_t row = (size_t)blockIdx.x * ROWS + rowl;
+    const size_t rowc = (size_t)blockIdx.x * ROWS + rowl, row = row0 + rowc;
     const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
     const double2 *src = W1 + row * NN;
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
@@ -228,18 +239,36 @@ __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ 
             v0[cc * T + k2] = src[16 * k2 + cc * T + j];
             v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
         }
+    // a8: the prolonged contribution of the coarser levels, fetched (from L2: the previous launch
+    // wrote it) while the row's spectrum is still on its way, so its latency hides behind the transform
+    const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
+    double ext[16];
+    if (b > 0) {
+        const double *Hc = hole_c + (size_t)(b - 1) * N * N * N;
+        const int pk = Q + z / 2, pj = Q + y / 2, sk = (z & 1) ? 1 : -1, sj = (y & 1) ? 1 : -1;
+        const double *h0 = Hc + ((size_t)pk * N + pj) * N, *h1 = Hc + ((size_t)(pk + sk) * N + (pj + sj)) * N;
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int x = j + T * r, pi = Q + x / 2, si = (x & 1) ? 1 : -1;
+            ext[r] = 0.75 * __ldcg(h0 + pi) + 0.25 * __ldcg(h1 + pi + si);
+        }
+    } else {
+#pragma unroll
+        for (int r = 0; r < 16; ++r) ext[r] = 0.0;
+    }
+
     double2 e[16], o[16];
     inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
     inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncWarp());
 
     const double scale = scale0 * exp2(-2.0 * b);   // dx_b^2 = dx0^2 / 4^b, exact
-    const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
     double *dphi = phi + row * N, *dh = hole + row * N;
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
         const int x = j + T * r;
-        dphi[x] = scale * (e[r].x + o[r].x);
-        if (rowring && in_ring1(x, N)) dh[x] = scale * (e[r].y + o[r].y);
+        const double re = scale * (e[r].x + o[r].x), im = scale * (e[r].y + o[r].y);
+        dphi[x] = b > 0 ? re + ext[r] : re;
+        if (rowring && in_ring1(x, N)) dh[x] = b > 0 ? im + ext[r] : im;
     }
 }
 
@@ -394,26 +423,6 @@ __global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_
                          : rho_f[((size_t)k * N + jx) * N + i];
             }
     rc_out[idx] = 0.125 * s;
-}
-
-// ===================== a8: prolongation + Eq. 14 sum, one level ====================
-// Hc = ext_{l-1} + Phi_hole^{l-1} on the coarse grid (valid on the cavity grown by one
-// cell).  Fine cell f: parent p = N/4 + f/2, sign s = +1 (f odd) / -1 (f even);
-// ext_l(f) = 3/4 Hc[p] + 1/4 Hc[p+s]  (Eq. 3-6); phi_l += ext_l  (Eq. 14);
-// hole_l += ext_l where the next level will need it.
-__global__ void k_prolong_sum(int N, int l, int L, const double *__restrict__ Hc, double *__restrict__ phi_l,
-                              double *__restrict__ hole_l)
-{
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= N * N * N) return;
-    const int fi = idx % N, fj = (idx / N) % N, fk = idx / (N * N);
-    const int Q = N / 4;
-    const int pk = Q + fk / 2, pj = Q + fj / 2, pi = Q + fi / 2;
-    const int sk = (fk & 1) ? 1 : -1, sj = (fj & 1) ? 1 : -1, si = (fi & 1) ? 1 : -1;
-    const double e = 0.75 * Hc[((size_t)pk * N + pj) * N + pi] +
-                     0.25 * Hc[((size_t)(pk + sk) * N + (pj + sj)) * N + (pi + si)];
-    phi_l[idx] += e;
-    if (l < L - 1 && in_ring1(fk, N) && in_ring1(fj, N) && in_ring1(fi, N)) hole_l[idx] += e;
 }
 
 // ============================ a0: Green's function ================================

@@ -40,6 +40,7 @@ struct cm_plan {
     int zconv_mode = 0;             // 2 = parity-split direct kernel
     bool zconv_tma = true;          // P3 through the TMA-fed persistent kernel (CM_ZCONV=direct selects the first version)
     CUtensorMap mapW, mapK;
+    int kernels_per_solve = 0;
     char err[512] = {0};
 };
 
@@ -74,19 +75,12 @@ template <int T> int set_attrs(cm_plan *p)
     return CM_OK;
 }
 
-// The five FFT passes for every level at once (steps a3-a7).
-template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev)
+// P3 for every level in one launch (step a5).
+template <int T> void launch_zconv(cm_plan *p, cudaStream_t s)
 {
     constexpr int N = 16 * T, NN = 2 * N;
     const int L = p->L;
-    const size_t rows = (size_t)L * N * N;
-    const unsigned gx = (unsigned)(rows / (kThreads / T));
-    const unsigned gy = (unsigned)((size_t)L * N * NN / (8 * (16 / T)));
     const unsigned gz = (unsigned)((size_t)NN * NN / (8 * (16 / T)) * L);
-    k_x_fwd<T><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
-    if (ev) cudaEventRecord(ev[2], s);
-    k_y_fwd<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
-    if (ev) cudaEventRecord(ev[3], s);
     if (p->zconv_mode == 2) {
         const size_t sm = sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T);
         const int ntile = NN * NN / (8 * (16 / T));
@@ -101,12 +95,31 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     } else {
         k_z_conv<T><<<gz, kThreads, smem_batch<T>(), s>>>(p->W2, p->Khat, p->tw, L);
     }
+}
+
+// The five FFT passes (steps a3-a7) with the prolongation + Eq. 14 sum (a8) folded into P5:
+// P1-P4 take every level in one launch; P5 runs level by level, coarse -> fine, because
+// level b adds the prolonged hole potentials of level b-1 (k_x_inv).
+template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev)
+{
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = 8 * (16 / T);
+    const int L = p->L;
+    const size_t planes = (size_t)L * N;
+    const double scale0 = -p->G * p->dx0 * p->dx0;
+    k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
+    if (ev) cudaEventRecord(ev[2], s);
+    k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    if (ev) cudaEventRecord(ev[3], s);
+    launch_zconv<T>(p, s);
     if (ev) cudaEventRecord(ev[4], s);
-    k_y_inv<T><<<gy, kThreads, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
+    k_y_inv<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
     if (ev) cudaEventRecord(ev[5], s);
-    k_x_inv<T><<<gx, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->tw, L, -p->G * p->dx0 * p->dx0);
+    const size_t lrows = (size_t)N * N;
+    const unsigned gl = (unsigned)((lrows + ROWS - 1) / ROWS);
+    for (int b = 0; b < L; ++b)
+        k_x_inv<T><<<gl, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, L, scale0, (size_t)b * lrows);
     if (ev) cudaEventRecord(ev[6], s);
-    p->launches += 5;
+    p->launches += 4 + L;
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
@@ -135,13 +148,7 @@ int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cu
         case 16: rcode = launch_passes<16>(p, rho, phi, s, ev); break;
     }
     if (rcode != CM_OK) return rcode;
-    // a8: prolongation + Eq. 14 sum, coarse -> fine
-    for (int l = 1; l < L; ++l) {
-        k_prolong_sum<<<(unsigned)((n3 + 255) / 256), 256, 0, s>>>(N, l, L, p->hole + n3 * (l - 1), phi + n3 * l,
-                                                                    p->hole + n3 * l);
-        p->launches++;
-    }
-    CM_CUDA(p, cudaGetLastError());
+    // a8 (prolongation + Eq. 14 sum) ran inside P5
     if (ev) cudaEventRecord(ev[7], s);
     return CM_OK;
 }
@@ -239,11 +246,6 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
 
     const size_t n = 2 * (size_t)N, n3 = (size_t)N * N * N, h3 = n3 / 8, L = (size_t)levels;
     int rc = CM_OK;
-    int ndev = 0;
-    if (cuda_fail(p, cudaGetDeviceCount(&ndev), "cudaGetDeviceCount") || ndev == 0) {
-        delete p;
-        return CM_ECUDA;
-    }
     if ((rc = dev_alloc(p, &p->W1, L * N * N * n)) == CM_OK &&
         (rc = dev_alloc(p, &p->W2, L * N * n * n)) == CM_OK &&
         (rc = dev_alloc(p, &p->Khat, n * n * n)) == CM_OK &&
@@ -293,8 +295,9 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         cm_plan_destroy(p);
         return rc;
     }
-    // number of kernels per solve: (L-1) restrictions + 5 passes + (L-1) prolongations
-    p->launches = 2 * (levels - 1) + 5;
+    // number of kernels per solve: (L-1) restrictions + P1..P4 + one P5 per level
+    p->kernels_per_solve = (levels - 1) + 4 + levels;
+    p->launches = p->kernels_per_solve;
     *out = p;
     return CM_OK;
 }
@@ -424,7 +427,7 @@ int cm_plan_set_G(cm_plan *p, double G)
 
 size_t cm_plan_workspace_bytes(const cm_plan *p) { return p ? p->bytes : 0; }
 
-int cm_plan_kernel_launches(const cm_plan *p) { return p ? 2 * (p->L - 1) + 5 : 0; }
+int cm_plan_kernel_launches(const cm_plan *p) { return p ? p->kernels_per_solve : 0; }
 
 int cm_debug_copy(cm_plan *p, int which, double *dst, size_t n_doubles, void *stream)
 {
