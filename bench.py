@@ -341,7 +341,8 @@ def run_ours(args) -> None:
         "frac": achieved / peaks["hbm_gbs"], "traffic": None, "peak_source": peaks["source"],
         "algorithmic_bytes_per_launch": alg[dom], "implemented_bytes_per_launch": impl[dom],
         "kernel_ms": stage_ms[dom], "per_pass": per_pass,
-        "aux_ms": {"restrict": round(stage_ms["restrict"], 4), "prolong_sum": round(stage_ms["prolong_sum"], 4)},
+        "aux_ms": {"restrict": round(stage_ms["restrict"], 4), "prolong_sum": round(stage_ms["prolong_sum"], 4),
+                   "note": "a8 (prolongation + Eq. 14 sum) runs inside P5_x_inv, one launch per level"},
         "stage_sum_ms": sum(stage_ms.values()),
         "whole_solve_alg_GBs": solve_alg_bytes / (ms_step * 1e-3) / 1e9,
         "whole_solve_frac": solve_alg_bytes / (ms_step * 1e-3) / 1e9 / peaks["hbm_gbs"],

@@ -93,7 +93,7 @@ int cm_potential_host(cm_plan *plan, const double *rho_host, double *phi_host, v
  * the stage durations in milliseconds to ms_host[0..6] (host):
  *   [0] restriction cascade (a1)   [1] P1 x forward   [2] P2 y forward
  *   [3] P3 z forward * K-hat * z inverse   [4] P4 y inverse   [5] P5 x inverse
- *   [6] prolongation + sum cascade (a8).
+ *   [6] prolongation + sum cascade (a8): folded into P5 (one launch per level), reported as ~0.
  * n_ms must be 7.  Results in phi_levels are identical to cm_potential's.
  */
 int cm_potential_profile(cm_plan *plan, const double *rho_levels, double *phi_levels, void *stream,

@@ -105,8 +105,6 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
 
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31, j = lane % T, pxl = lane / T;
     const int pen = w * C::PPW + pxl, bx = pen >> 3, px = pen & 7;
-    const size_t zs = (size_t)NN * NN;
-
     if ((int)blockIdx.x >= ngroups) return;
     const int my_groups = (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
     const int ntiles = my_groups * L;
@@ -198,13 +196,13 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
         if (b == L - 1 && t + 1 < ntiles) { __syncthreads(); if (tid == 0) issue_k(g + (int)gridDim.x); }
 #else
         double2 e[16];
+        if (b == 0) {   // a new group: its K-hat tile was requested during the previous group's last tile
+            mbar_wait(bar_k, ph_k);
+            ph_k ^= 1;
+        }
         {
             double2 v[16];
             fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncX());
-            if (b == 0) {
-                mbar_wait(bar_k, ph_k);
-                ph_k ^= 1;
-            }
             kmul(v, 0);
             inv_half<T, 0, Lay, true>(v, e, j, ex_p, tws, SyncX());
         }
@@ -212,10 +210,6 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
             double2 v[16], o[16];
             fwd_half<T, 1, Lay, true>(a, v, j, ex_p, tws, SyncX());
             kmul(v, 1);
-            if (b == L - 1 && t + 1 < ntiles) {   // last use of this group's K-hat tile
-                __syncthreads();
-                if (tid == 0) issue_k(g + (int)gridDim.x);
-            }
             inv_half<T, 1, Lay, true>(v, o, j, ex_p, tws, SyncX());
 #pragma unroll
             for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
@@ -224,6 +218,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
         // stage the output tile in the (now idle) exchange buffer with the box layout of the
         // input stage, then one thread hands it to the TMA unit: full 128-byte rows to L2.
         __syncthreads();   // every warp is done with its exchanges
+        if (tid == 0 && b == L - 1 && t + 1 < ntiles) issue_k(g + (int)gridDim.x);   // last use of this group's K-hat tile is over
         {
             unsigned char *out_p = sbase + C::OFF_EX + bx * (N * 128);
 #pragma unroll
