@@ -67,16 +67,32 @@ struct SyncWarp  { __device__ __forceinline__ void operator()() const { __syncwa
 struct TwGlobal {
     const double2 *__restrict__ tw;
     int j;
+    static constexpr bool RECUR = false;
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return __ldg(&tw[j * (2 * k1 + P)]); }
+    __device__ __forceinline__ double2 step() const { return make_double2(1.0, 0.0); }
 };
+// P3 is bound by the shared-memory data pipe (profiles/r01b), not by fp64: only the even-k1 twiddles are
+// read from the table; an odd one is the even one before it times rho = w_2N^{2j}, kept in registers
+// (one extra rounding, ~1e-16).
 template <int T> struct TwShared {
     const double2 *base;   // table + j
+    double2 rho;           // w_2N^{2 j}
+    static constexpr bool RECUR = true;
 #ifndef ABL_NOTW
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return base[(2 * k1 + P) * T]; }
 #else
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return make_double2(0.6 + k1, 0.8 - P); }
 #endif
+    __device__ __forceinline__ double2 step() const { return rho; }
 };
+
+// twiddle w_2N^{j (2 k1 + P)} for k1 = 0..15 in turn; `prev` carries the last even-k1 value
+template <int P, class Tw> __device__ __forceinline__ double2 tw_next(const Tw &tw, int k1, double2 &prev)
+{
+    if (Tw::RECUR && (k1 & 1)) return (P == 0 && k1 == 1) ? tw.step() : cmul(prev, tw.step());
+    prev = tw.template get<P>(k1);
+    return prev;
+}
 
 // ---- half transforms ---------------------------------------------------------------
 // Forward, parity P: a[r] = input element n = j + T r (r < 16).  On return
@@ -93,9 +109,10 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
     Dft<16, -1>::run(b);
     if (T > 1) {
         if (PRE) sync();
+        double2 twp = make_double2(1.0, 0.0);
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
-            if (k1 > 0 || P) b[k1] = cmul(b[k1], tw.template get<P>(k1));
+            if (k1 > 0 || P) b[k1] = cmul(b[k1], tw_next<P>(tw, k1, twp));
 #ifndef ABL_NOEX
             sm[k1 * Lay::RS + j] = b[k1];
 #endif
@@ -139,6 +156,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
 #ifndef ABL_NOEX
         sync();
 #endif
+        double2 twp = make_double2(1.0, 0.0);
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
 #ifndef ABL_NOEX
@@ -146,7 +164,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
 #else
             o[k1] = v[k1];
 #endif
-            if (k1 > 0 || P) o[k1] = cmulc(o[k1], tw.template get<P>(k1));
+            if (k1 > 0 || P) o[k1] = cmulc(o[k1], tw_next<P>(tw, k1, twp));
         }
     } else {
 #pragma unroll

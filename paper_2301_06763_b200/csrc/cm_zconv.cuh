@@ -147,7 +147,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
 #ifdef ZC_TWGLOBAL
     const TwGlobal tws{tw, j};
 #else
-    const TwShared<T> tws{tw_s + j};
+    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j]};
 #endif
 #ifdef ZC_SYNCBLOCK
     using SyncX = SyncBlock;
@@ -201,12 +201,12 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
             ph_k ^= 1;
         }
         {
-            double2 v[16];
-            fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncX());
-            kmul(v, 0);
-            inv_half<T, 0, Lay, true>(v, e, j, ex_p, tws, SyncX());
-        }
-        {
+            {
+                double2 v[16];
+                fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncX());
+                kmul(v, 0);
+                inv_half<T, 0, Lay, true>(v, e, j, ex_p, tws, SyncX());
+            }
             double2 v[16], o[16];
             fwd_half<T, 1, Lay, true>(a, v, j, ex_p, tws, SyncX());
             kmul(v, 1);
@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(256, 2) k_z_conv_ps(double2 *__restrict__ W2, 
 #endif
     for (int i = threadIdx.x; i < 32 * T; i += 256) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
     __syncthreads();
-    const TwShared<T> tws{tw_s + j};
+    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j]};
 
     double2 o[16];
 #ifdef ABL_NOCOMPUTE
