@@ -41,6 +41,7 @@ def _assert_parity(got, ref, tol=TOL):
         worst = max(worst, e)
         assert e <= tol, f"level {l}: rel err {e:.3e} > {tol}"
     assert np.abs(got - ref).max() / np.abs(ref).max() <= tol
+    print(f"PARITY worst per-level rel err {worst:.3e} over {ref.shape[0]} levels of {ref.shape[1]}^3")
     return worst
 
 
