@@ -10,6 +10,9 @@ from .cm_oracle import (build, lib, I0, restrict, field_direct, field_fft, green
                         prolong, solve, solve_points, leaf_direct, num_threads,
                         fft1d, dft_naive, field_direct_at)
 
-__all__ = ["build", "lib", "I0", "restrict", "field_direct", "field_fft", "green_hat",
+from .cm_accel import acceleration, ghost_value, child_mean, padded_level
+
+__all__ = ["acceleration", "ghost_value", "child_mean", "padded_level",
+           "build", "lib", "I0", "restrict", "field_direct", "field_fft", "green_hat",
            "prolong", "solve", "solve_points", "leaf_direct", "num_threads",
            "fft1d", "dft_naive", "field_direct_at"]

@@ -83,3 +83,32 @@ def gaussian_phi(s, A, sigma, G=1.0):
     s = np.asarray(s, float)
     M = A * (2.0 * np.pi) ** 1.5 * sigma ** 3
     return -G * M * erf(s / (np.sqrt(2.0) * sigma)) / s
+
+
+def sphere_g(x, y, z, R, rho, centre=(0.0, 0.0, 0.0), G=1.0):
+    """|g| of a homogeneous sphere: 4/3 pi G rho r inside, G M / r^2 outside."""
+    r = np.sqrt((x - centre[0]) ** 2 + (y - centre[1]) ** 2 + (z - centre[2]) ** 2)
+    M = 4.0 / 3.0 * np.pi * R ** 3 * rho
+    with np.errstate(divide="ignore"):
+        return np.where(r <= R, 4.0 / 3.0 * np.pi * G * rho * r, G * M / (r * r))
+
+
+def ellipsoid_g(x, y, z, semi_axes, rho, G=1.0):
+    """Acceleration components of Chandrasekhar's homogeneous ellipsoid: the derivative of
+    ellipsoid_phi (the lambda-dependence drops out because the integrand vanishes at u = lambda):
+    g_i = -2 pi G rho a1 a2 a3 x_i int_lam^inf du / ((a_i^2+u) sqrt(prod (a_j^2+u)))."""
+    x, y, z = np.broadcast_arrays(np.asarray(x, float), np.asarray(y, float), np.asarray(z, float))
+    shape = x.shape
+    xs = (x.ravel(), y.ravel(), z.ravel())
+    a2 = np.asarray(semi_axes, float) ** 2
+    amax2 = a2.max()
+    lam = _ellipsoid_lambda(xs[0] ** 2, xs[1] ** 2, xs[2] ** 2, a2)
+    acc = [np.zeros_like(lam) for _ in range(3)]
+    for w, wt in zip(_GL_X, _GL_W):
+        u = lam + amax2 * (1.0 / (w * w) - 1.0)
+        d = (a2[0] + u, a2[1] + u, a2[2] + u)
+        delta = np.sqrt(d[0] * d[1] * d[2])
+        for i in range(3):
+            acc[i] += wt * (2.0 * amax2 / w ** 3) / (d[i] * delta)
+    pref = -2.0 * np.pi * G * rho * np.sqrt(a2.prod())
+    return tuple((pref * xs[i] * acc[i]).reshape(shape) for i in range(3))
