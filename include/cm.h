@@ -99,6 +99,23 @@ int cm_potential_host(cm_plan *plan, const double *rho_host, double *phi_host, v
 int cm_potential_profile(cm_plan *plan, const double *rho_levels, double *phi_levels, void *stream,
                          float *ms_host, int n_ms);
 
+/*
+ * Gravitational acceleration g = -grad Phi on every level, from potentials
+ * that cm_potential produced (or any potentials laid out the same way):
+ *   six-point central stencil, g_x = -(Phi[i+1] - Phi[i-1]) / (2 dx_l)          (Eq. 8);
+ *   method A (Eq. A.1): a neighbour outside a fine grid (level l > 0) is the ghost value
+ *     interpolated from level l-1 with Eq. 3-6 (L64-L76): 3/4 Phi_c[p] + 1/4 Phi_c[p+s];
+ *   method B (Eq. A.2): a neighbour that lies under the finer grid is the arithmetic
+ *     mean of the potentials of its 8 children on level l+1;
+ *   outer boundary of level 0 (the method has no boundary values, L164): second-order one-sided
+ *     difference (paper-silent).
+ *   phi_levels : device, const, [levels][N][N][N] fp64, 16-byte aligned.
+ *   g_levels   : device, [levels][3][N][N][N] fp64 (component x, y, z), overwritten; must not
+ *                alias phi_levels.
+ * Enqueues two kernels on `stream` and returns; does not need cm_green_precompute.
+ */
+int cm_acceleration(cm_plan *plan, const double *phi_levels, double *g_levels, void *stream);
+
 /* Release the plan and everything it owns.  NULL is accepted. */
 int cm_plan_destroy(cm_plan *plan);
 

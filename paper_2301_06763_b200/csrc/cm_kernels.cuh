@@ -500,4 +500,85 @@ __global__ void k_green_permute(const double2 *__restrict__ Gm, double *__restri
     }
 }
 
+// ===================== f-1: gravitational acceleration on the nested mesh ==================
+// g = -grad Phi by the six-point stencil (Eq. 8); a neighbour the level cannot
+// supply comes from the parent level through Eq. 3-6 (method A, Eq. A.1), a neighbour
+// that lies under the finer grid is the mean of its 8 children (method B, Eq. A.2),
+// and the outer boundary of level 0 uses the second-order one-sided difference.
+
+// pbar[l][ck][cj][ci] = mean of the 8 children (level l+1) of cavity cell (N/4 + c*) of level l.
+__global__ void k_child_mean(int N, int L, const double *__restrict__ phi, double *__restrict__ pbar)
+{
+    const int H = N / 2;
+    const size_t h3 = (size_t)H * H * H, n3 = (size_t)N * N * N;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)(L - 1) * h3) return;
+    const int l = (int)(idx / h3);
+    const size_t r = idx - (size_t)l * h3;
+    const int ci = (int)(r % H), cj = (int)((r / H) % H), ck = (int)(r / ((size_t)H * H));
+    const double *f = phi + (size_t)(l + 1) * n3;
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            const double2 v = *reinterpret_cast<const double2 *>(f + ((size_t)(2 * ck + c) * N + (2 * cj + b)) * N + 2 * ci);
+            s += v.x;
+            s += v.y;
+        }
+    pbar[idx] = s / 8.0;
+}
+
+// value of level l at (k, j, i), any ONE of which may be -1 or N
+struct AccelField {
+    const double *phi_l, *phi_c, *pbar_l;   // this level, its parent (nullptr on level 0), children means (nullptr on the finest)
+    int N;
+    __device__ __forceinline__ double core(int k, int j, int i) const
+    {
+        const int Q = N / 4, H = N / 2;
+        if (pbar_l && in_cavity1(k, N) && in_cavity1(j, N) && in_cavity1(i, N))
+            return pbar_l[((size_t)(k - Q) * H + (j - Q)) * H + (i - Q)];
+        return phi_l[((size_t)k * N + j) * N + i];
+    }
+    // ghost beyond the face: along axis `ax` the index f is -1 or N
+    __device__ __forceinline__ double ghost(int k, int j, int i, int ax) const
+    {
+        if (!phi_c) {   // level 0: 3 Phi[0] - 3 Phi[1] + Phi[2] makes the central formula the one-sided one
+            const int f = ax == 0 ? i : (ax == 1 ? j : k);
+            const int d = f < 0 ? 1 : -1, e0 = f + d;
+            const int di = ax == 0 ? d : 0, dj = ax == 1 ? d : 0, dk = ax == 2 ? d : 0;
+            const int i0 = ax == 0 ? e0 : i, j0 = ax == 1 ? e0 : j, k0 = ax == 2 ? e0 : k;
+            return (3.0 * core(k0, j0, i0) - 3.0 * core(k0 + dk, j0 + dj, i0 + di)) + core(k0 + 2 * dk, j0 + 2 * dj, i0 + 2 * di);
+        }
+        const int Q = N / 4;
+        // floor(f/2) and parity for f = -1: parent Q-1, odd
+        const int pk = Q + ((k + 2) >> 1) - 1, pj = Q + ((j + 2) >> 1) - 1, pi = Q + ((i + 2) >> 1) - 1;
+        const int sk = (k & 1) ? 1 : -1, sj = (j & 1) ? 1 : -1, si = (i & 1) ? 1 : -1;
+        return 0.75 * phi_c[((size_t)pk * N + pj) * N + pi] + 0.25 * phi_c[((size_t)(pk + sk) * N + (pj + sj)) * N + (pi + si)];
+    }
+    __device__ __forceinline__ double at(int k, int j, int i, int ax) const
+    {
+        const int f = ax == 0 ? i : (ax == 1 ? j : k);
+        return (f < 0 || f >= N) ? ghost(k, j, i, ax) : core(k, j, i);
+    }
+};
+
+// one thread per cell; g layout [L][3][N][N][N] (component x, y, z)
+__global__ void __launch_bounds__(256) k_accel(int N, int L, double dx0, const double *__restrict__ phi,
+                                               const double *__restrict__ pbar, double *__restrict__ g)
+{
+    const size_t n3 = (size_t)N * N * N, h3 = n3 / 8;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)L * n3) return;
+    const int l = (int)(idx / n3);
+    const size_t r = idx - (size_t)l * n3;
+    const int i = (int)(r % N), j = (int)((r / N) % N), k = (int)(r / ((size_t)N * N));
+    AccelField F{phi + (size_t)l * n3, l > 0 ? phi + (size_t)(l - 1) * n3 : nullptr, l < L - 1 ? pbar + (size_t)l * h3 : nullptr, N};
+    const double two_dx = 2.0 * (dx0 * exp2(-(double)l));
+    double *gl = g + (size_t)l * 3 * n3 + r;
+    gl[0] = -(F.at(k, j, i + 1, 0) - F.at(k, j, i - 1, 0)) / two_dx;
+    gl[n3] = -(F.at(k, j + 1, i, 1) - F.at(k, j - 1, i, 1)) / two_dx;
+    gl[2 * n3] = -(F.at(k + 1, j, i, 2) - F.at(k - 1, j, i, 2)) / two_dx;
+}
+
 }  // namespace cmk

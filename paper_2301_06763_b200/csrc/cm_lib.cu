@@ -27,7 +27,7 @@ struct cm_plan {
     int N = 0, L = 0, T = 0;
     double dx0 = 0, G = 1.0;
     double2 *W1 = nullptr, *W2 = nullptr, *tw = nullptr;
-    double *Khat = nullptr, *rc = nullptr, *hole = nullptr;
+    double *Khat = nullptr, *rc = nullptr, *hole = nullptr, *pbar = nullptr;
     double *stage_rho = nullptr, *stage_phi = nullptr;
     size_t bytes = 0;
     bool green_ready = false;
@@ -251,6 +251,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         (rc = dev_alloc(p, &p->Khat, n * n * n)) == CM_OK &&
         (rc = dev_alloc(p, &p->rc, (L > 1 ? L - 1 : 1) * h3)) == CM_OK &&
         (rc = dev_alloc(p, &p->hole, L * n3)) == CM_OK &&
+        (rc = dev_alloc(p, &p->pbar, (L > 1 ? L - 1 : 1) * h3)) == CM_OK &&
         (rc = dev_alloc(p, &p->tw, n)) == CM_OK) {
         // twiddles w_2N^m = exp(-2 pi i m / 2N), computed in long double on the host
         std::vector<double2> tw(n);
@@ -400,6 +401,22 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
     return CM_OK;
 }
 
+int cm_acceleration(cm_plan *p, const double *phi, double *g, void *stream)
+{
+    if (!p || !phi || !g) return CM_EINVAL;
+    if (((uintptr_t)phi & 15) || ((uintptr_t)g & 15)) return CM_EINVAL;
+    const size_t n3 = (size_t)p->N * p->N * p->N, tot = (size_t)p->L * n3, h3 = n3 / 8;
+    if ((phi <= g && g < phi + tot) || (g <= phi && phi < g + 3 * tot)) return CM_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (p->L > 1) {
+        const size_t cnt = (size_t)(p->L - 1) * h3;
+        k_child_mean<<<(unsigned)((cnt + 255) / 256), 256, 0, s>>>(p->N, p->L, phi, p->pbar);
+    }
+    k_accel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(p->N, p->L, p->dx0, phi, p->pbar, g);
+    CM_CUDA(p, cudaGetLastError());
+    return CM_OK;
+}
+
 int cm_plan_destroy(cm_plan *p)
 {
     if (!p) return CM_OK;
@@ -410,6 +427,7 @@ int cm_plan_destroy(cm_plan *p)
     cudaFree(p->Khat);
     cudaFree(p->rc);
     cudaFree(p->hole);
+    cudaFree(p->pbar);
     cudaFree(p->tw);
     cudaFree(p->stage_rho);
     cudaFree(p->stage_phi);
