@@ -563,22 +563,71 @@ struct AccelField {
     }
 };
 
-// one thread per cell; g layout [L][3][N][N][N] (component x, y, z)
-__global__ void __launch_bounds__(256) k_accel(int N, int L, double dx0, const double *__restrict__ phi,
+// Two x-adjacent cells per thread, marching kAccelZ planes in z with the z-neighbours kept in
+// registers; a CTA is a (TY rows) x (TX pairs) tile so that the y- and x-neighbours are L1 hits.
+// g layout [L][3][N][N][N] (component x, y, z).  A step whose stencil touches neither a face of
+// the grid nor the cavity takes the fast path; the others go through AccelField.  HBM-bound:
+// 8 B read + 24 B written per cell.
+constexpr int kAccelZ = 16;
+
+// the general (face / cavity) case of one pair of cells, kept out of line so that the streaming
+// loop of k_accel stays small in registers
+__device__ __noinline__ void accel_pair_general(const AccelField F, int k, int j, int i, double inv, double2 &gx,
+                                                double2 &gy, double2 &gz)
+{
+    const double c0 = F.at(k, j, i, 0), c1 = F.at(k, j, i + 1, 0);
+    gx = make_double2(-(c1 - F.at(k, j, i - 1, 0)) * inv, -(F.at(k, j, i + 2, 0) - c0) * inv);
+    gy = make_double2(-(F.at(k, j + 1, i, 1) - F.at(k, j - 1, i, 1)) * inv,
+                      -(F.at(k, j + 1, i + 1, 1) - F.at(k, j - 1, i + 1, 1)) * inv);
+    gz = make_double2(-(F.at(k + 1, j, i, 2) - F.at(k - 1, j, i, 2)) * inv,
+                      -(F.at(k + 1, j, i + 1, 2) - F.at(k - 1, j, i + 1, 2)) * inv);
+}
+
+__global__ void __launch_bounds__(256) k_accel(int N, int L, int TX, int TY, double dx0, const double *__restrict__ phi,
                                                const double *__restrict__ pbar, double *__restrict__ g)
 {
-    const size_t n3 = (size_t)N * N * N, h3 = n3 / 8;
-    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (size_t)L * n3) return;
-    const int l = (int)(idx / n3);
-    const size_t r = idx - (size_t)l * n3;
-    const int i = (int)(r % N), j = (int)((r / N) % N), k = (int)(r / ((size_t)N * N));
-    AccelField F{phi + (size_t)l * n3, l > 0 ? phi + (size_t)(l - 1) * n3 : nullptr, l < L - 1 ? pbar + (size_t)l * h3 : nullptr, N};
-    const double two_dx = 2.0 * (dx0 * exp2(-(double)l));
-    double *gl = g + (size_t)l * 3 * n3 + r;
-    gl[0] = -(F.at(k, j, i + 1, 0) - F.at(k, j, i - 1, 0)) / two_dx;
-    gl[n3] = -(F.at(k, j + 1, i, 1) - F.at(k, j - 1, i, 1)) / two_dx;
-    gl[2 * n3] = -(F.at(k + 1, j, i, 2) - F.at(k - 1, j, i, 2)) / two_dx;
+    const size_t n3 = (size_t)N * N * N, h3 = n3 / 8, nn = (size_t)N * N;
+    const int Q = N / 4;
+    const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
+    const int ntx = (N / 2) / TX, nty = N / TY, nz = N / kAccelZ;
+    int bid = blockIdx.x;
+    const int bx = bid % ntx; bid /= ntx;
+    const int by = bid % nty; bid /= nty;
+    const int bz = bid % nz;
+    const int l = bid / nz;
+    const int i = 2 * (bx * TX + tx), j = by * TY + ty, k0 = bz * kAccelZ;
+    const double inv = 1.0 / (2.0 * (dx0 * exp2(-(double)l)));
+    const double *pl = phi + (size_t)l * n3;
+    const bool has_cav = l < L - 1;
+    const AccelField F{pl, l > 0 ? phi + (size_t)(l - 1) * n3 : nullptr, has_cav ? pbar + (size_t)l * h3 : nullptr, N};
+    const bool inner_ji = j >= 1 && j <= N - 2 && i >= 2 && i <= N - 4;
+    const bool cav_ji = has_cav && j >= Q - 1 && j <= 3 * Q && i >= Q - 2 && i <= 3 * Q;
+    const size_t rji = (size_t)j * N + i;
+    double2 zm = make_double2(0.0, 0.0), c = *reinterpret_cast<const double2 *>(pl + (size_t)k0 * nn + rji);
+    if (k0 > 0) zm = *reinterpret_cast<const double2 *>(pl + (size_t)(k0 - 1) * nn + rji);
+#pragma unroll 2
+    for (int kk = 0; kk < kAccelZ; ++kk) {
+        const int k = k0 + kk;
+        const size_t r = (size_t)k * nn + rji;
+        double2 zp = make_double2(0.0, 0.0);
+        if (k + 1 < N) zp = *reinterpret_cast<const double2 *>(pl + r + nn);
+        double2 gx, gy, gz;
+        if (inner_ji && k >= 1 && k <= N - 2 && !(cav_ji && k >= Q - 1 && k <= 3 * Q)) {
+            const double xm = pl[r - 1], xp = pl[r + 2];
+            const double2 ym = *reinterpret_cast<const double2 *>(pl + r - N), yp = *reinterpret_cast<const double2 *>(pl + r + N);
+            gx = make_double2(-(c.y - xm) * inv, -(xp - c.x) * inv);
+            gy = make_double2(-(yp.x - ym.x) * inv, -(yp.y - ym.y) * inv);
+            gz = make_double2(-(zp.x - zm.x) * inv, -(zp.y - zm.y) * inv);
+        } else {
+            accel_pair_general(F, k, j, i, inv, gx, gy, gz);
+        }
+        double *gl = g + (size_t)l * 3 * n3 + r;
+        __stcs(reinterpret_cast<double2 *>(gl), gx);
+        __stcs(reinterpret_cast<double2 *>(gl + n3), gy);
+        __stcs(reinterpret_cast<double2 *>(gl + 2 * n3), gz);
+        zm = c;
+        c = zp;
+    }
 }
 
 }  // namespace cmk

@@ -412,7 +412,11 @@ int cm_acceleration(cm_plan *p, const double *phi, double *g, void *stream)
         const size_t cnt = (size_t)(p->L - 1) * h3;
         k_child_mean<<<(unsigned)((cnt + 255) / 256), 256, 0, s>>>(p->N, p->L, phi, p->pbar);
     }
-    k_accel<<<(unsigned)((tot + 255) / 256), 256, 0, s>>>(p->N, p->L, p->dx0, phi, p->pbar, g);
+    {
+        const int N = p->N, TX = N / 2 < 32 ? N / 2 : 32, TY = (256 / TX) < N ? 256 / TX : N;
+        const unsigned grid = (unsigned)((size_t)p->L * (N / kAccelZ) * (N / TY) * ((N / 2) / TX));
+        k_accel<<<grid, TX * TY, 0, s>>>(N, p->L, TX, TY, p->dx0, phi, p->pbar, g);
+    }
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
