@@ -563,12 +563,11 @@ struct AccelField {
     }
 };
 
-// Two x-adjacent cells per thread, marching kAccelZ planes in z with the z-neighbours kept in
+// Two x-adjacent cells per thread, marching ZCH planes in z with the z-neighbours kept in
 // registers; a CTA is a (TY rows) x (TX pairs) tile so that the y- and x-neighbours are L1 hits.
 // g layout [L][3][N][N][N] (component x, y, z).  A step whose stencil touches neither a face of
 // the grid nor the cavity takes the fast path; the others go through AccelField.  HBM-bound:
 // 8 B read + 24 B written per cell.
-constexpr int kAccelZ = 16;
 
 // the general (face / cavity) case of one pair of cells, kept out of line so that the streaming
 // loop of k_accel stays small in registers
@@ -583,19 +582,19 @@ __device__ __noinline__ void accel_pair_general(const AccelField F, int k, int j
                       -(F.at(k + 1, j, i + 1, 2) - F.at(k - 1, j, i + 1, 2)) * inv);
 }
 
-__global__ void __launch_bounds__(256) k_accel(int N, int L, int TX, int TY, double dx0, const double *__restrict__ phi,
+__global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, int ZCH, double dx0, const double *__restrict__ phi,
                                                const double *__restrict__ pbar, double *__restrict__ g)
 {
     const size_t n3 = (size_t)N * N * N, h3 = n3 / 8, nn = (size_t)N * N;
     const int Q = N / 4;
     const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
-    const int ntx = (N / 2) / TX, nty = N / TY, nz = N / kAccelZ;
+    const int ntx = (N / 2) / TX, nty = N / TY, nz = N / ZCH;
     int bid = blockIdx.x;
     const int bx = bid % ntx; bid /= ntx;
     const int by = bid % nty; bid /= nty;
     const int bz = bid % nz;
     const int l = bid / nz;
-    const int i = 2 * (bx * TX + tx), j = by * TY + ty, k0 = bz * kAccelZ;
+    const int i = 2 * (bx * TX + tx), j = by * TY + ty, k0 = bz * ZCH;
     const double inv = 1.0 / (2.0 * (dx0 * exp2(-(double)l)));
     const double *pl = phi + (size_t)l * n3;
     const bool has_cav = l < L - 1;
@@ -606,7 +605,7 @@ __global__ void __launch_bounds__(256) k_accel(int N, int L, int TX, int TY, dou
     double2 zm = make_double2(0.0, 0.0), c = *reinterpret_cast<const double2 *>(pl + (size_t)k0 * nn + rji);
     if (k0 > 0) zm = *reinterpret_cast<const double2 *>(pl + (size_t)(k0 - 1) * nn + rji);
 #pragma unroll 2
-    for (int kk = 0; kk < kAccelZ; ++kk) {
+    for (int kk = 0; kk < ZCH; ++kk) {
         const int k = k0 + kk;
         const size_t r = (size_t)k * nn + rji;
         double2 zp = make_double2(0.0, 0.0);

@@ -414,8 +414,9 @@ int cm_acceleration(cm_plan *p, const double *phi, double *g, void *stream)
     }
     {
         const int N = p->N, TX = N / 2 < 32 ? N / 2 : 32, TY = (256 / TX) < N ? 256 / TX : N;
-        const unsigned grid = (unsigned)((size_t)p->L * (N / kAccelZ) * (N / TY) * ((N / 2) / TX));
-        k_accel<<<grid, TX * TY, 0, s>>>(N, p->L, TX, TY, p->dx0, phi, p->pbar, g);
+        const int ZCH = N >= 256 ? 16 : (N >= 128 ? 8 : (N >= 64 ? 4 : 2));   // planes a thread marches: enough CTAs at small N
+        const unsigned grid = (unsigned)((size_t)p->L * (N / ZCH) * (N / TY) * ((N / 2) / TX));
+        k_accel<<<grid, TX * TY, 0, s>>>(N, p->L, TX, TY, ZCH, p->dx0, phi, p->pbar, g);
     }
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
