@@ -60,6 +60,8 @@ template <int T> struct LayRow {
 
 struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
 struct SyncWarp  { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
+// the kThreads compute threads of a CTA that also carries a scheduler warp (cm_fused.cuh)
+struct SyncCompute { __device__ __forceinline__ void operator()() const { asm volatile("bar.sync 1, 128;" ::: "memory"); } };
 
 // ---- twiddle sources ------------------------------------------------------------------
 // w_2N^{j (2 k1 + P)}: from the global table (read-only path) or from a per-CTA shared copy
@@ -180,17 +182,14 @@ __device__ __forceinline__ bool in_ring1(int v, int N) { return v >= N / 4 - 1 &
 // ================================ P1: x forward ====================================
 // One row (b, z, y) per group of T threads (j fastest).  Reads N reals, forms the complex
 // pair field (step a2, never materialised), writes 2N complex slots.
+// body: thread (rowl, j) of a CTA transforms global row `row` (b, z, y) and writes its 2N slots to `dst`
 template <int T>
-__global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ rho, const double *__restrict__ rc,
-                                                    double2 *__restrict__ W1, const double2 *__restrict__ tw, int L,
-                                                    size_t row0)
+__device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const double *__restrict__ rc, double2 *dst,
+                                           const double2 *__restrict__ tw, int L, size_t row, double2 *smem)
 {
-    // row0: first global row (b, z, y) of this launch
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, H = N / 2, Q = N / 4;
+    constexpr int N = 16 * T, ROWS = kThreads / T, H = N / 2, Q = N / 4;
     using Lay = LayRow<T>;
-    extern __shared__ double2 smem[];
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
-    const size_t rowc = (size_t)blockIdx.x * ROWS + rowl, row = row0 + rowc;
     const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
     const bool finest = (b == L - 1);
     const bool rowcav = !finest && in_cavity1(z, N) && in_cavity1(y, N);
@@ -206,7 +205,6 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ r
         a[r] = make_double2(re, (finest || cav) ? 0.0 : re);
     }
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
-    double2 *dst = W1 + row * NN;
     {
         double2 v[16];
         fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncWarp());
@@ -223,6 +221,18 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ r
 #pragma unroll
             for (int k2 = 0; k2 < T; ++k2) dst[N + 16 * k2 + cc * T + j] = v[cc * T + k2];
     }
+}
+
+template <int T>
+__global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ rho, const double *__restrict__ rc,
+                                                    double2 *__restrict__ W1, const double2 *__restrict__ tw, int L,
+                                                    size_t row0)
+{
+    // row0: first global row (b, z, y) of this launch
+    constexpr int NN = 32 * T, ROWS = kThreads / T;
+    extern __shared__ double2 smem[];
+    const size_t row = row0 + (size_t)blockIdx.x * ROWS + threadIdx.x / T;
+    x_fwd_body<T>(rho, rc, W1 + row * NN, tw, L, row, smem);
 }
 
 // ====================== P5: x inverse + a8 (prolongation, Eq. 14) ==================
@@ -295,27 +305,23 @@ __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ 
 // g = tid / (8 T).  A CTA covers 8 * G adjacent batch positions, G = 16 / T.
 
 // ================================ P2: y forward ====================================
-template <int T>
-__global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ W1, double2 *__restrict__ W2,
-                                                    const double2 *__restrict__ tw)
+// body: the CTA transforms PEN = 8 * (16/T) adjacent sx columns of one (b, z) plane; src/dst point at
+// this thread's column (sx) of the plane's W1 rows / W2 rows.  COHERENT: read W1 through L2 only
+// (ld.global.cg) — needed when another CTA of the same kernel produced it (cm_fused.cuh).
+template <int T, bool COHERENT, class Sync = SyncBlock>
+__device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, const double2 *__restrict__ tw, double2 *smem)
 {
     constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
     using Lay = LayBatch<T>;
-    extern __shared__ double2 smem[];
     const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
-    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
-    const size_t bz = q / NN;
-    const int sx = (int)(q % NN);
-    const double2 *src = W1 + bz * N * NN + sx;
-    double2 *dst = W2 + bz * NN * NN + sx;
     double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
 
     double2 a[16];
 #pragma unroll
-    for (int r = 0; r < 16; ++r) a[r] = src[(size_t)(j + T * r) * NN];
+    for (int r = 0; r < 16; ++r) a[r] = COHERENT ? __ldcg(src + (size_t)(j + T * r) * NN) : src[(size_t)(j + T * r) * NN];
     {
         double2 v[16];
-        fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncBlock());
+        fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, Sync());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
@@ -323,12 +329,25 @@ __global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ 
     }
     {
         double2 v[16];
-        fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, SyncBlock());
+        fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, Sync());
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
             for (int k2 = 0; k2 < T; ++k2) dst[(size_t)(N + 16 * k2 + cc * T + j) * NN] = v[cc * T + k2];
     }
+}
+
+template <int T>
+__global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ W1, double2 *__restrict__ W2,
+                                                    const double2 *__restrict__ tw)
+{
+    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    extern __shared__ double2 smem[];
+    const int tid = threadIdx.x, px = tid & 7, g = tid / (8 * T);
+    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
+    const size_t bz = q / NN;
+    const int sx = (int)(q % NN);
+    y_fwd_body<T, false>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
 }
 
 // ================================ P4: y inverse ====================================

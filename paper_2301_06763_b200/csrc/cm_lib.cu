@@ -11,6 +11,7 @@
 #include "../../include/cm.h"
 #include "cm_kernels.cuh"
 #include "cm_zconv.cuh"
+#include "cm_fused.cuh"
 
 namespace {
 
@@ -41,6 +42,10 @@ struct cm_plan {
     bool zconv_tma = true;          // P3 through the TMA-fed persistent kernel (CM_ZCONV=direct selects the first version)
     CUtensorMap mapW, mapK;
     int kernels_per_solve = 0;
+    bool fused_fwd = false;         // P1+P2 as one persistent kernel (cm_fused.cuh), N >= 128, CM_FUSE=1
+    int fuse_R = 0, fuse_LAG = 0, fuse_grid = 0;
+    cmk::FusedCtl *ctl = nullptr;
+    size_t ctl_bytes = 0;
     char err[512] = {0};
 };
 
@@ -71,6 +76,8 @@ template <int T> int set_attrs(cm_plan *p)
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_ps<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T))));
+    CM_CUDA(p, cudaFuncSetAttribute(k_xy_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>())));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
     return CM_OK;
 }
@@ -106,9 +113,17 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     const int L = p->L;
     const size_t planes = (size_t)L * N;
     const double scale0 = -p->G * p->dx0 * p->dx0;
-    k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
-    if (ev) cudaEventRecord(ev[2], s);
-    k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    if (p->fused_fwd) {
+        // P1 and P2 interleave inside one persistent kernel: reported together under P2
+        if (ev) cudaEventRecord(ev[2], s);
+        cudaMemsetAsync(p->ctl, 0, p->ctl_bytes, s);
+        const size_t sm = smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>();
+        k_xy_fwd<T><<<p->fuse_grid, kThreads + 32, sm, s>>>(rho, p->rc, p->W1, p->W2, p->tw, L, p->ctl, p->fuse_R, p->fuse_LAG);
+    } else {
+        k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
+        if (ev) cudaEventRecord(ev[2], s);
+        k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    }
     if (ev) cudaEventRecord(ev[3], s);
     launch_zconv<T>(p, s);
     if (ev) cudaEventRecord(ev[4], s);
@@ -119,7 +134,7 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     for (int b = 0; b < L; ++b)
         k_x_inv<T><<<gl, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, L, scale0, (size_t)b * lrows);
     if (ev) cudaEventRecord(ev[6], s);
-    p->launches += 4 + L;
+    p->launches += (p->fused_fwd ? 3 : 4) + L;
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
@@ -272,6 +287,29 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
             rc = CM_ECUDA;
     }
     if (rc == CM_OK) {
+        // fused P1+P2: ring and lag in planes from the number of tickets in flight (cm_fused.cuh)
+        const char *ef = std::getenv("CM_FUSE");
+        p->fused_fwd = (N >= 128) && (ef && ef[0] == '1');   // off by default: correct, 40 % fewer DRAM bytes, but latency-bound
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        const int T = N / 16, per = N >= 128 ? N / (kThreads / T) + 2 * N / (8 * (16 / T)) : 1;
+        p->fuse_grid = 2 * sms;
+        const int span = (p->fuse_grid + per - 1) / per;
+        p->fuse_LAG = span + 1;
+        p->fuse_R = p->fuse_LAG + span + 2;
+        const char *el = std::getenv("CM_FUSE_LAG"), *er = std::getenv("CM_FUSE_R"), *eg = std::getenv("CM_FUSE_GRID");
+        if (el) p->fuse_LAG = std::atoi(el);
+        if (er) p->fuse_R = std::atoi(er);
+        if (eg) p->fuse_grid = std::atoi(eg);
+        if (p->fuse_R <= p->fuse_LAG) p->fuse_R = p->fuse_LAG + 1;
+        if ((size_t)p->fuse_R > L * N) p->fused_fwd = false;
+        p->ctl_bytes = sizeof(FusedCtl) + 2 * L * N * sizeof(unsigned);
+        void *q = nullptr;
+        if (cuda_fail(p, cudaMalloc(&q, p->ctl_bytes), "cudaMalloc(ctl)")) rc = CM_ECUDA;
+        p->ctl = (cmk::FusedCtl *)q;
+    }
+    if (rc == CM_OK) {
         const char *zc = std::getenv("CM_ZCONV");
         p->zconv_tma = !(zc && std::strcmp(zc, "direct") == 0);
         if (zc && std::strcmp(zc, "ps") == 0) p->zconv_mode = 2;
@@ -297,7 +335,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         return rc;
     }
     // number of kernels per solve: (L-1) restrictions + P1..P4 + one P5 per level
-    p->kernels_per_solve = (levels - 1) + 4 + levels;
+    p->kernels_per_solve = (levels - 1) + (p->fused_fwd ? 3 : 4) + levels;
     p->launches = p->kernels_per_solve;
     *out = p;
     return CM_OK;
@@ -433,6 +471,7 @@ int cm_plan_destroy(cm_plan *p)
     cudaFree(p->rc);
     cudaFree(p->hole);
     cudaFree(p->pbar);
+    cudaFree(p->ctl);
     cudaFree(p->tw);
     cudaFree(p->stage_rho);
     cudaFree(p->stage_phi);

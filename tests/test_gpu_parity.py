@@ -273,3 +273,25 @@ def test_G_scales_linearly_and_error_codes():
         pkg.cm_potential(h, t.data_ptr() + 8, torch.empty_like(t).data_ptr(), 0)   # misaligned
     assert ei.value.code == pkg.CM_EINVAL
     pkg.cm_plan_destroy(h)
+
+
+def test_fused_forward_kernel_is_bit_identical_to_the_two_pass_path(monkeypatch):
+    """CM_FUSE=1 runs P1+P2 as one persistent kernel with a W1 ring in L2 (cm_fused.cuh; not the default,
+    DESIGN.md §6).  Same arithmetic in the same order: the potentials must be bit-identical."""
+    pkg = _pkg()
+    N, L = 128, 3
+    rho = np.random.default_rng(9).random((L, N, N, N))
+    d = torch.from_numpy(rho).cuda()
+    monkeypatch.delenv("CM_FUSE", raising=False)
+    p0 = pkg.Plan(N, L, 2.0 / N)
+    a = p0.potential(d).clone()
+    k0 = p0.kernel_launches
+    p0.close()
+    monkeypatch.setenv("CM_FUSE", "1")
+    p1 = pkg.Plan(N, L, 2.0 / N)
+    assert p1.kernel_launches == k0 - 1
+    b = p1.potential(d).clone()
+    b2 = p1.potential(d).clone()          # second solve: the control block is reset by the graph
+    p1.close()
+    torch.cuda.synchronize()
+    assert torch.equal(a, b) and torch.equal(a, b2)

@@ -119,7 +119,7 @@ def _cfg5(N, L):
         amp = np.where(k2 > 0, k2 ** (-0.75), 0.0)          # |k|^-3/2  => P(k) ~ k^-3
     for l in range(L):
         w = level_rng(5, l).standard_normal((N, N, N))
-        d = np.fft.irfftn(np.fft.rfftn(w) * amp, s=(N, N, N))
+        d = np.fft.irfftn(np.fft.rfftn(w) * amp, s=(N, N, N), axes=(0, 1, 2))
         d = (d - d.mean()) / d.std()
         X, Y, Z = _grid(N, l)
         out[l] = np.exp(1.5 * d) / (X * X + Y * Y + Z * Z)
