@@ -421,10 +421,44 @@ def run_ours(args) -> None:
         "cpu_baseline": cpu,
         "acceleration": accel,
     }
+    if args.cufft_ref and world == 1:
+        plan.close()
+        del rho, phi
+        torch.cuda.empty_cache()
+        line["cufft_dense_reference"] = cufft_dense_reference(N, L, torch)
     print(json.dumps(line), flush=True)
     plan.close()
     if dist is not None:
         dist.destroy_process_group()
+
+
+def cufft_dense_reference(N: int, L: int, torch) -> dict:
+    """Context only (--cufft-ref): the paper's own GPU scheme on this GPU — per field a dense
+    zero-padded (2N)^3 cuFFT D2Z, a pointwise multiply and a Z2D, here through torch.fft; restriction,
+    interpolation and assembly (host-side in the paper) are not included.  Never linked into libcm."""
+    n = 2 * N
+    rho = torch.rand(N, N, N, dtype=torch.float64, device="cuda")
+    khat = torch.rand(n, n, n // 2 + 1, dtype=torch.float64, device="cuda")
+
+    def field():
+        pad = torch.zeros(n, n, n, dtype=torch.float64, device="cuda")
+        pad[:N, :N, :N] = rho
+        f = torch.fft.rfftn(pad)
+        f *= khat
+        return torch.fft.irfftn(f, s=(n, n, n))[:N, :N, :N]
+
+    for _ in range(2):
+        field()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(5):
+        field()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 5
+    return {"ms_per_field": ms, "ms_per_solve": (2 * L - 1) * ms, "fields": 2 * L - 1,
+            "what": "torch.fft rfftn/irfftn (cuFFT) on the dense (2N)^3 + multiply, FFT part of the paper's scheme only"}
 
 
 def main() -> None:
@@ -435,6 +469,7 @@ def main() -> None:
     ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cufft-ref", action="store_true", help="also time the paper's dense cuFFT scheme (context)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

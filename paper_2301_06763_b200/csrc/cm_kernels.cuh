@@ -305,6 +305,9 @@ __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ 
 // g = tid / (8 T).  A CTA covers 8 * G adjacent batch positions, G = 16 / T.
 
 // ================================ P2: y forward ====================================
+// (min-blocks choices are measured: at N = 256 P2 and P4 gain 3-5 % when compiled for 3 CTAs per
+// SM (168 registers); at smaller N P2 is best left to ptxas (178 registers) and P4 with a floor of 2 CTAs,
+// which lets ptxas use 230 registers: -15 % at N = 128)
 // body: the CTA transforms PEN = 8 * (16/T) adjacent sx columns of one (b, z) plane; src/dst point at
 // this thread's column (sx) of the plane's W1 rows / W2 rows.  COHERENT: read W1 through L2 only
 // (ld.global.cg) — needed when another CTA of the same kernel produced it (cm_fused.cuh).
@@ -350,9 +353,23 @@ __global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ 
     y_fwd_body<T, false>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
 }
 
+// the same kernel compiled for 3 CTAs per SM (168 registers): used at N = 256
+template <int T>
+__global__ void __launch_bounds__(kThreads, 3) k_y_fwd_occ3(const double2 *__restrict__ W1, double2 *__restrict__ W2,
+                                                    const double2 *__restrict__ tw)
+{
+    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    extern __shared__ double2 smem[];
+    const int tid = threadIdx.x, px = tid & 7, g = tid / (8 * T);
+    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
+    const size_t bz = q / NN;
+    const int sx = (int)(q % NN);
+    y_fwd_body<T, false>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
+}
+
 // ================================ P4: y inverse ====================================
 template <int T>
-__global__ void __launch_bounds__(kThreads) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
+__global__ void __launch_bounds__(kThreads, T == 16 ? 3 : 2) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
                                                     const double2 *__restrict__ tw)
 {
     constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;

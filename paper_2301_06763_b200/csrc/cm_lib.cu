@@ -72,11 +72,13 @@ template <int T> int set_attrs(cm_plan *p)
     CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_occ3<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_ps<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T))));
-    CM_CUDA(p, cudaFuncSetAttribute(k_xy_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if constexpr (T >= 8)
+        CM_CUDA(p, cudaFuncSetAttribute(k_xy_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>())));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
     return CM_OK;
@@ -113,16 +115,22 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     const int L = p->L;
     const size_t planes = (size_t)L * N;
     const double scale0 = -p->G * p->dx0 * p->dx0;
+    bool fused_done = false;
+    if constexpr (T >= 8) {
     if (p->fused_fwd) {
+        fused_done = true;
         // P1 and P2 interleave inside one persistent kernel: reported together under P2
         if (ev) cudaEventRecord(ev[2], s);
         cudaMemsetAsync(p->ctl, 0, p->ctl_bytes, s);
         const size_t sm = smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>();
         k_xy_fwd<T><<<p->fuse_grid, kThreads + 32, sm, s>>>(rho, p->rc, p->W1, p->W2, p->tw, L, p->ctl, p->fuse_R, p->fuse_LAG);
-    } else {
+    }
+    }
+    if (!fused_done) {
         k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
         if (ev) cudaEventRecord(ev[2], s);
-        k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+        if (T == 16) k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+        else k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     }
     if (ev) cudaEventRecord(ev[3], s);
     launch_zconv<T>(p, s);
