@@ -98,7 +98,9 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s)
         k_z_conv_ps<T><<<gz, 256, sm, s>>>(p->W2, p->Khat, p->tw, L, lo);
     } else if (p->zconv_tma) {
         const int ngroups = NN * NN / ZConvCfg<T>::PEN;
-        int grid = ngroups < 2 * p->num_sms ? ngroups : 2 * p->num_sms;
+        // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
+        const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
+        int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
         if (p->zconv_grid > 0 && p->zconv_grid < grid) grid = p->zconv_grid;
         k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->mapK, p->W2, p->tw, L, ngroups);
     } else {

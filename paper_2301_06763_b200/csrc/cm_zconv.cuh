@@ -105,9 +105,31 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
 
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31, j = lane % T, pxl = lane / T;
     const int pen = w * C::PPW + pxl, bx = pen >> 3, px = pen & 7;
-    if ((int)blockIdx.x >= ngroups) return;
-    const int my_groups = (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-    const int ntiles = my_groups * L;
+    // Tiles (g, b) in g-major order.  Large grids: CTA c takes groups c, c + gridDim, ... (at any moment the
+    // grid works on adjacent 128-byte columns: DRAM page locality).  N <= 64: there are only 1-2 groups per CTA,
+    // so the flat tile list is cut into gridDim equal ranges instead (balance; the data is L2-resident anyway).
+    constexpr bool FLAT = (T <= 4);
+    int t0 = 0, ntiles;
+    if (FLAT) {
+        const long long total = (long long)ngroups * L;
+        t0 = (int)(total * blockIdx.x / gridDim.x);
+        ntiles = (int)(total * (blockIdx.x + 1) / gridDim.x) - t0;
+        if (ntiles <= 0) return;
+    } else {
+        if ((int)blockIdx.x >= ngroups) return;
+        const int my_groups = (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+        ntiles = my_groups * L;
+    }
+    auto tile_of = [&](int t, int &g, int &b) {
+        if (FLAT) {
+            g = (t0 + t) / L;
+            b = (t0 + t) - g * L;
+        } else {
+            const int gi = t / L;
+            b = t - gi * L;
+            g = (int)blockIdx.x + gi * (int)gridDim.x;
+        }
+    };
 
     auto issue_in = [&](int g, int b) {
         // the stage was last touched through the generic proxy (LDS): order those accesses before
@@ -137,8 +159,10 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
     for (int i = tid; i < 32 * T; i += kThreads) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
     __syncthreads();
     if (tid == 0) {
-        issue_k((int)blockIdx.x);
-        issue_in((int)blockIdx.x, 0);
+        int g0, b0;
+        tile_of(0, g0, b0);
+        issue_k(g0);
+        issue_in(g0, b0);
     }
 
     const unsigned char *in_p = sbase + C::OFF_IN + bx * (N * 128);
@@ -157,8 +181,9 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
     uint32_t ph_in = 0, ph_k = 0;
 
     for (int t = 0; t < ntiles; ++t) {
-        const int gi = t / L, b = t - gi * L;
-        const int g = (int)blockIdx.x + gi * (int)gridDim.x;
+        int g, b, gn = 0, bn = 0;
+        tile_of(t, g, b);
+        if (t + 1 < ntiles) tile_of(t + 1, gn, bn);
 
         mbar_wait(bar_in, ph_in);
         ph_in ^= 1;
@@ -170,10 +195,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
         }
         if (tid == 0) tma_store_wait_read();   // the previous tile's output has left the exchange/out buffer
         __syncthreads();   // every thread holds its part of the tile: the stage may be refilled
-        if (tid == 0 && t + 1 < ntiles) {
-            if (b + 1 < L) issue_in(g, b + 1);
-            else issue_in(g + (int)gridDim.x, 0);
-        }
+        if (tid == 0 && t + 1 < ntiles) issue_in(gn, bn);
 
         auto kmul = [&](double2(&v)[16], int P) {
 #pragma unroll
@@ -187,16 +209,8 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
                 }
         };
 
-#ifdef ZC_NOCOMPUTE
         double2 e[16];
-        if (b == 0) { mbar_wait(bar_k, ph_k); ph_k ^= 1; }
-#pragma unroll
-        for (int r = 0; r < 16; ++r) e[r] = a[r];
-        kmul(e, 0);
-        if (b == L - 1 && t + 1 < ntiles) { __syncthreads(); if (tid == 0) issue_k(g + (int)gridDim.x); }
-#else
-        double2 e[16];
-        if (b == 0) {   // a new group: its K-hat tile was requested during the previous group's last tile
+        if (t == 0 || b == 0) {   // a new group: its K-hat tile was requested during the previous group's last tile
             mbar_wait(bar_k, ph_k);
             ph_k ^= 1;
         }
@@ -214,11 +228,10 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
 #pragma unroll
             for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
         }
-#endif
         // stage the output tile in the (now idle) exchange buffer with the box layout of the
         // input stage, then one thread hands it to the TMA unit: full 128-byte rows to L2.
         __syncthreads();   // every warp is done with its exchanges
-        if (tid == 0 && b == L - 1 && t + 1 < ntiles) issue_k(g + (int)gridDim.x);   // last use of this group's K-hat tile is over
+        if (tid == 0 && t + 1 < ntiles && gn != g) issue_k(gn);   // last use of this group's K-hat tile is over
         {
             unsigned char *out_p = sbase + C::OFF_EX + bx * (N * 128);
 #pragma unroll

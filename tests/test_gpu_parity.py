@@ -295,3 +295,29 @@ def test_fused_forward_kernel_is_bit_identical_to_the_two_pass_path(monkeypatch)
     p1.close()
     torch.cuda.synchronize()
     assert torch.equal(a, b) and torch.equal(a, b2)
+
+
+def test_maximum_level_count():
+    """levels = 32 (the ABI's maximum) at N = 16: dx_l spans 2^-31, the -G dx_l^2 scale 2^-62 — still exact
+    powers of two; parity against the FFT oracle on every level."""
+    N, L = 16, 32
+    rng = np.random.default_rng(32)
+    rho = rng.random((L, N, N, N)) * (4.0 ** np.arange(L))[:, None, None, None]   # keep rho dx^2 comparable
+    got, plan = _solve_gpu(rho, 2.0 / N)
+    ref = oracle.solve(rho, 2.0 / N, method="fft")
+    _assert_parity(got, ref)
+    plan.close()
+
+
+def test_single_level_at_the_largest_grid():
+    """N = 256, levels = 1 (no cavity, no prolongation): sampled outputs against direct sums."""
+    N = 256
+    rng = np.random.default_rng(256)
+    rho = rng.random((1, N, N, N))
+    got, plan = _solve_gpu(rho, 2.0 / N)
+    targets = [(0, 0, 0, 0), (0, 255, 255, 255), (0, 17, 200, 100), (0, 128, 0, 255)]
+    ref = oracle.solve_points(rho, 2.0 / N, targets)
+    scale = np.abs(got).max()
+    for t, r in zip(targets, ref):
+        assert abs(got[t] - r) <= TOL * scale, (t, got[t], r)
+    plan.close()
