@@ -415,7 +415,7 @@ def run_ours(args) -> None:
         "clocks": clocks,
         "e2e": {"value": world * cells / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                 "h2d_bytes_per_step": rho_h.numel() * 8, "d2h_bytes_per_step": phi_h.numel() * 8,
-                "api": "cm_potential_host (pinned host rho -> device -> solve -> pinned host phi)"},
+                "api": "cm_potential_host (pinned host rho -> device -> solve -> pinned host phi; level pipeline for N >= 128)"},
         "gpu_launches": args.steps * launches_per_step,
         "roofline": roofline,
         "cpu_baseline": cpu,

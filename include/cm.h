@@ -83,7 +83,11 @@ int cm_potential(cm_plan *plan, const double *rho_levels, double *phi_levels, vo
  * Same computation with HOST buffers (pinned memory recommended): copies
  * rho_host -> device staging, runs cm_potential, copies the result into phi_host
  * and synchronises `stream` before returning.  Staging buffers belong to the plan
- * and are allocated on first use.
+ * and are allocated on first use.  For N >= 128 the call is a level pipeline: rho is
+ * copied finest level first on a plan-owned copy stream, each level's projection (a1)
+ * and passes P1-P4 run under the copy of the next level, P5 + a8 run coarse -> fine at
+ * the end and each level's Phi leaves for the host under the next level's P5.  Same
+ * kernels, bit-identical results; for N < 128 it is copy - cm_potential - copy.
  */
 int cm_potential_host(cm_plan *plan, const double *rho_host, double *phi_host, void *stream);
 

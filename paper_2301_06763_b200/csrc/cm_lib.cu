@@ -33,7 +33,8 @@ struct cm_plan {
     size_t bytes = 0;
     bool green_ready = false;
     bool use_graph = true;
-    cudaStream_t cap_stream = nullptr;
+    cudaStream_t cap_stream = nullptr, copy_stream = nullptr;
+    std::vector<cudaEvent_t> ev_level;   // cm_potential_host's pipeline: [0,32) level arrived, [32,64) level's Phi ready, [64] start
     std::vector<GraphEntry> graphs;
     int launches = 0;
     int num_sms = 148;
@@ -85,10 +86,10 @@ template <int T> int set_attrs(cm_plan *p)
 }
 
 // P3 for every level in one launch (step a5).
-template <int T> void launch_zconv(cm_plan *p, cudaStream_t s)
+// levels [b0, b0 + L) of W2 (the TMA kernel only; the alternates take every level)
+template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
 {
     constexpr int N = 16 * T, NN = 2 * N;
-    const int L = p->L;
     const unsigned gz = (unsigned)((size_t)NN * NN / (8 * (16 / T)) * L);
     if (p->zconv_mode == 2) {
         const size_t sm = sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T);
@@ -102,7 +103,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s)
         const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
         int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
         if (p->zconv_grid > 0 && p->zconv_grid < grid) grid = p->zconv_grid;
-        k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->mapK, p->W2, p->tw, L, ngroups);
+        k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->mapK, p->W2, p->tw, L, ngroups, b0);
     } else {
         k_z_conv<T><<<gz, kThreads, smem_batch<T>(), s>>>(p->W2, p->Khat, p->tw, L);
     }
@@ -135,7 +136,7 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
         else k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     }
     if (ev) cudaEventRecord(ev[3], s);
-    launch_zconv<T>(p, s);
+    launch_zconv<T>(p, s, 0, L);
     if (ev) cudaEventRecord(ev[4], s);
     k_y_inv<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
     if (ev) cudaEventRecord(ev[5], s);
@@ -147,6 +148,37 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     p->launches += (p->fused_fwd ? 3 : 4) + L;
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
+}
+
+// One level's P1..P4 / P5 on their own (cm_potential_host's pipeline): the same kernels on the level's
+// slices of W1 / W2; P3 then runs with a one-level range, so K-hat is read once per level (irrelevant there:
+// that path is bound by the host link).
+template <int T> void level_p1_to_p4(cm_plan *p, const double *rho, cudaStream_t s, int l)
+{
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = 8 * (16 / T);
+    const size_t lrows = (size_t)N * N;
+    double2 *w1 = p->W1 + (size_t)l * lrows * NN, *w2 = p->W2 + (size_t)l * N * NN * NN;
+    k_x_fwd<T><<<(unsigned)(lrows / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows);
+    k_y_fwd<T><<<(unsigned)((size_t)N * NN / PEN), kThreads, smem_batch<T>(), s>>>(w1, w2, p->tw);
+    launch_zconv<T>(p, s, l, 1);
+    k_y_inv<T><<<(unsigned)((size_t)N * NN / PEN), kThreads, smem_batch<T>(), s>>>(w2, w1, p->tw);
+}
+template <int T> void level_p5(cm_plan *p, double *phi, cudaStream_t s, int l)
+{
+    constexpr int N = 16 * T, ROWS = kThreads / T;
+    const size_t lrows = (size_t)N * N;
+    k_x_inv<T><<<(unsigned)((lrows + ROWS - 1) / ROWS), kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, p->L,
+                                                                                   -p->G * p->dx0 * p->dx0, (size_t)l * lrows);
+}
+void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int l, bool p5)
+{
+    switch (p->T) {
+        case 1: p5 ? level_p5<1>(p, phi, s, l) : level_p1_to_p4<1>(p, rho, s, l); break;
+        case 2: p5 ? level_p5<2>(p, phi, s, l) : level_p1_to_p4<2>(p, rho, s, l); break;
+        case 4: p5 ? level_p5<4>(p, phi, s, l) : level_p1_to_p4<4>(p, rho, s, l); break;
+        case 8: p5 ? level_p5<8>(p, phi, s, l) : level_p1_to_p4<8>(p, rho, s, l); break;
+        case 16: p5 ? level_p5<16>(p, phi, s, l) : level_p1_to_p4<16>(p, rho, s, l); break;
+    }
 }
 
 // ev (optional): 8 events; ev[0] start, ev[1] after a1, ev[2..6] after P1..P5, ev[7] after a8
@@ -432,7 +464,7 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
 {
     if (!p || !rho_host || !phi_host) return CM_EINVAL;
     if (!p->green_ready) return CM_ENOTREADY;
-    const size_t tot = (size_t)p->L * p->N * p->N * p->N;
+    const size_t n3 = (size_t)p->N * p->N * p->N, tot = (size_t)p->L * n3;
     if (!p->stage_rho) {
         size_t keep = p->bytes;
         int rc = dev_alloc(p, &p->stage_rho, tot);
@@ -441,10 +473,51 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
         if (rc != CM_OK) return rc;
     }
     cudaStream_t s = (cudaStream_t)stream;
-    CM_CUDA(p, cudaMemcpyAsync(p->stage_rho, rho_host, tot * sizeof(double), cudaMemcpyHostToDevice, s));
-    const int rc = cm_potential(p, p->stage_rho, p->stage_phi, stream);
-    if (rc != CM_OK) return rc;
-    CM_CUDA(p, cudaMemcpyAsync(phi_host, p->stage_phi, tot * sizeof(double), cudaMemcpyDeviceToHost, s));
+    if (p->N < 128 || !p->zconv_tma || p->zconv_mode == 2) {
+        // small grids are launch-bound, not link-bound: one copy in, the graph, one copy out
+        CM_CUDA(p, cudaMemcpyAsync(p->stage_rho, rho_host, tot * sizeof(double), cudaMemcpyHostToDevice, s));
+        const int rc = cm_potential(p, p->stage_rho, p->stage_phi, stream);
+        if (rc != CM_OK) return rc;
+        CM_CUDA(p, cudaMemcpyAsync(phi_host, p->stage_phi, tot * sizeof(double), cudaMemcpyDeviceToHost, s));
+        CM_CUDA(p, cudaStreamSynchronize(s));
+        return CM_OK;
+    }
+    // Level pipeline (N >= 128: the host link is the bound).  rho arrives finest level first on a copy
+    // stream; as soon as level l is there its projection onto level l-1 (a1) and its P1..P4 run, under the
+    // copy of the next level.  P5 + a8 must go coarse -> fine, so it starts when level 0 is through, and
+    // every level's Phi leaves for the host while the next level's P5 runs.
+    const int L = p->L;
+    const size_t h3 = n3 / 8;
+    if (!p->copy_stream) {
+        CM_CUDA(p, cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking));
+        p->ev_level.resize(2 * 32 + 1, nullptr);
+        for (auto &e : p->ev_level) CM_CUDA(p, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    }
+    cudaEvent_t *ev_in = p->ev_level.data(), *ev_out = ev_in + 32, ev_start = p->ev_level[64];
+    CM_CUDA(p, cudaEventRecord(ev_start, s));                       // work already queued on s comes first
+    CM_CUDA(p, cudaStreamWaitEvent(p->copy_stream, ev_start, 0));
+    for (int l = L - 1; l >= 0; --l) {
+        CM_CUDA(p, cudaMemcpyAsync(p->stage_rho + l * n3, rho_host + l * n3, n3 * sizeof(double), cudaMemcpyHostToDevice,
+                                   p->copy_stream));
+        CM_CUDA(p, cudaEventRecord(ev_in[l], p->copy_stream));
+    }
+    for (int l = L - 1; l >= 0; --l) {
+        CM_CUDA(p, cudaStreamWaitEvent(s, ev_in[l], 0));
+        if (l < L - 1) {                                            // rc[l] = projection of level l+1 (a1)
+            const double *rc_f = (l + 1 < L - 1) ? p->rc + h3 * (l + 1) : nullptr;
+            k_restrict<<<(unsigned)((h3 + 255) / 256), 256, 0, s>>>(p->N, l + 1, L, p->stage_rho + n3 * (l + 1), rc_f, p->rc + h3 * l);
+        }
+        dispatch_level(p, p->stage_rho, p->stage_phi, s, l, false);
+    }
+    for (int l = 0; l < L; ++l) {
+        dispatch_level(p, p->stage_rho, p->stage_phi, s, l, true);
+        CM_CUDA(p, cudaEventRecord(ev_out[l], s));
+        CM_CUDA(p, cudaStreamWaitEvent(p->copy_stream, ev_out[l], 0));
+        CM_CUDA(p, cudaMemcpyAsync(phi_host + l * n3, p->stage_phi + l * n3, n3 * sizeof(double), cudaMemcpyDeviceToHost,
+                                   p->copy_stream));
+    }
+    CM_CUDA(p, cudaGetLastError());
+    CM_CUDA(p, cudaStreamSynchronize(p->copy_stream));
     CM_CUDA(p, cudaStreamSynchronize(s));
     return CM_OK;
 }
@@ -475,6 +548,9 @@ int cm_plan_destroy(cm_plan *p)
     if (!p) return CM_OK;
     destroy_graphs(p);
     if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    for (auto e : p->ev_level)
+        if (e) cudaEventDestroy(e);
     cudaFree(p->W1);
     cudaFree(p->W2);
     cudaFree(p->Khat);

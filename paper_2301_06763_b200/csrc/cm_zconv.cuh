@@ -8,6 +8,7 @@
 // Why this shape (profiles/r01a_ncu_full_config5.md): the first k_z_conv was neither
 // DRAM- nor fp64-bound; its 8 warps/SM stalled on the tile load, on K-hat loads issued in
 // the middle of the dependency chain and on CTA-wide barriers.  Here
+//   (the launch covers levels b0 .. b0 + L - 1: all of them in cm_potential, one in cm_potential_host's pipeline)
 //   * a CTA is persistent and walks tiles (g, b): g = a group of PEN adjacent (sy,sx)
 //     pencils, b = level.  All L levels of a group run back to back so the group's
 //     K-hat tile is fetched ONCE (TMA, 64B-swizzled) and stays in shared memory;
@@ -91,7 +92,7 @@ template <int T> struct ZConvCfg {
 template <int T>
 __global__ void __launch_bounds__(kThreads, 2)
 k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapK,
-             double2 *__restrict__ W2, const double2 *__restrict__ tw, int L, int ngroups)
+             double2 *__restrict__ W2, const double2 *__restrict__ tw, int L, int ngroups, int b0)
 {
     using C = ZConvCfg<T>;
     constexpr int N = C::N, NN = C::NN, PEN = C::PEN, NBOX = C::NBOX;
@@ -139,7 +140,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
         mbar_expect_tx(bar_in, C::IN_BYTES);
 #pragma unroll
         for (int q = 0; q < NBOX; ++q)
-            tma_load_2d(s0 + C::OFF_IN + q * (N * 128), &mapW, 2 * (g * PEN + 8 * q), b * N, bar_in);
+            tma_load_2d(s0 + C::OFF_IN + q * (N * 128), &mapW, 2 * (g * PEN + 8 * q), (b0 + b) * N, bar_in);
     };
     auto issue_k = [&](int g) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -249,7 +250,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
 #ifndef ZC_NOSTORE
 #pragma unroll
             for (int q = 0; q < NBOX; ++q)
-                tma_store_2d(&mapW, 2 * (g * PEN + 8 * q), b * N, s0 + C::OFF_EX + q * (N * 128));
+                tma_store_2d(&mapW, 2 * (g * PEN + 8 * q), (b0 + b) * N, s0 + C::OFF_EX + q * (N * 128));
             tma_store_commit();
 #endif
         }

@@ -233,9 +233,12 @@ def test_repeat_solves_are_bit_identical_and_graph_cache_handles_new_buffers():
     plan.close()
 
 
-def test_host_buffer_entry_point_matches_device_entry_point():
+@pytest.mark.parametrize("N,L", [(32, 2), (128, 4)])
+def test_host_buffer_entry_point_matches_device_entry_point(N, L):
+    """N >= 128 takes cm_potential_host's level pipeline (copies under compute, P1..P4 level by level, K-hat
+    tile per level): the same kernels on the same data, so the potentials are bit-identical to cm_potential's;
+    called twice to check that the pipeline's events and staging are re-usable."""
     pkg = _pkg()
-    N, L = 32, 2
     rng = np.random.default_rng(10)
     rho = torch.from_numpy(rng.random((L, N, N, N))).pin_memory()
     plan = pkg.Plan(N, L, 2.0 / N)
@@ -243,6 +246,8 @@ def test_host_buffer_entry_point_matches_device_entry_point():
     pd = plan.potential(rho.cuda())
     torch.cuda.synchronize()
     assert torch.equal(ph, pd.cpu())
+    ph2 = plan.potential_host(rho)
+    assert torch.equal(ph2, ph)
     plan.close()
 
 
