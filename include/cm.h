@@ -120,6 +120,23 @@ int cm_potential_profile(cm_plan *plan, const double *rho_levels, double *phi_le
  */
 int cm_acceleration(cm_plan *plan, const double *phi_levels, double *g_levels, void *stream);
 
+/*
+ * The modified ("dipole") convolution method over every pair of neighbouring grids (
+ * PAPER.md:L282-L288 Eq. 15, L426-L433 Eq. B.1-B.2).  The original method lets a coarse grid see the
+ * finer grid's mass only through its projection, which cancels dipole moments; here, for every pair
+ * n : n+1, the fine grid is expanded to the physical size of the coarse one (a doubled grid of (2N)^3
+ * cells of the fine size, zero outside the fine grid), its potential is found by the same convolution
+ * on a (4N)^3 padded mesh, reduced to the coarse grid (mean of the 8 fine-size cells of a coarse cell)
+ * and added to the potential of the coarse grid with a cavity:
+ *     Phi(Omega^n) = Phi_hole^n + reduce(Phi_dbl^{n+1}) + sum_{k<n} tilde Phi_hole^k   (n not the finest)
+ *     Phi(Omega^n) = Phi^n + sum_{k<n} tilde Phi_hole^k                               (the finest grid)
+ * Arguments and conventions as cm_potential.  N <= 128 (the doubled grid must be a supported size);
+ * CM_EINVAL otherwise.  The first call creates the doubled-grid plan (its K-hat: 8 (2N)^3 bytes) and
+ * synchronises the device once; later calls only enqueue.  Cost: one extra (2N)^3 single-level
+ * convolution per pair (the paper: x4 on CPUs, x2 with GPUs, L433).
+ */
+int cm_potential_modified(cm_plan *plan, const double *rho_levels, double *phi_levels, void *stream);
+
 /* Release the plan and everything it owns.  NULL is accepted. */
 int cm_plan_destroy(cm_plan *plan);
 

@@ -17,7 +17,7 @@ CM_OK, CM_EINVAL, CM_ENOMEM, CM_ECUDA, CM_ENOTREADY = 0, -1, -2, -3, -4
 CM_BUF_RESTRICTED, CM_BUF_HOLE, CM_BUF_KHAT = 0, 1, 2
 
 EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potential_host", "cm_potential_profile",
-           "cm_acceleration",
+           "cm_acceleration", "cm_potential_modified",
            "cm_plan_destroy",
            "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
            "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error"]
@@ -42,6 +42,7 @@ def lib() -> C.CDLL:
     L.cm_potential_host.argtypes = [vp, vp, vp, vp]
     L.cm_potential_profile.argtypes = [vp, vp, vp, vp, C.POINTER(C.c_float), C.c_int]
     L.cm_acceleration.argtypes = [vp, vp, vp, vp]
+    L.cm_potential_modified.argtypes = [vp, vp, vp, vp]
     L.cm_plan_destroy.argtypes = [vp]
     L.cm_plan_set_G.argtypes = [vp, C.c_double]
     L.cm_plan_workspace_bytes.argtypes = [vp]
@@ -89,6 +90,10 @@ def cm_potential_profile(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0)
     ms = (C.c_float * 7)()
     _check(lib().cm_potential_profile(plan, rho_ptr, phi_ptr, stream, ms, 7), plan)
     return [float(v) for v in ms]
+
+
+def cm_potential_modified(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0) -> None:
+    _check(lib().cm_potential_modified(plan, rho_ptr, phi_ptr, stream), plan)
 
 
 def cm_acceleration(plan: int, phi_ptr: int, g_ptr: int, stream: int = 0) -> None:
@@ -148,6 +153,17 @@ class Plan:
         self._check_tensor(phi, "cuda")
         s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
         cm_potential(self._h, rho.data_ptr(), phi.data_ptr(), s)
+        return phi
+
+    def potential_modified(self, rho, phi=None, stream=None):
+        """Modified (dipole) method over neighbouring pairs, Eq. B.1-B.2 (cm_potential_modified)."""
+        import torch
+        self._check_tensor(rho, "cuda")
+        if phi is None:
+            phi = torch.empty_like(rho)
+        self._check_tensor(phi, "cuda")
+        s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
+        cm_potential_modified(self._h, rho.data_ptr(), phi.data_ptr(), s)
         return phi
 
     def acceleration(self, phi, g=None, stream=None):

@@ -185,7 +185,8 @@ __device__ __forceinline__ bool in_ring1(int v, int N) { return v >= N / 4 - 1 &
 // body: thread (rowl, j) of a CTA transforms global row `row` (b, z, y) and writes its 2N slots to `dst`
 template <int T>
 __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const double *__restrict__ rc, double2 *dst,
-                                           const double2 *__restrict__ tw, int L, size_t row, double2 *smem)
+                                           const double2 *__restrict__ tw, int L, size_t row, double2 *smem,
+                                           const double *__restrict__ rho_im = nullptr)
 {
     constexpr int N = 16 * T, ROWS = kThreads / T, H = N / 2, Q = N / 4;
     using Lay = LayRow<T>;
@@ -202,7 +203,9 @@ __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const
         const int x = j + T * r;
         const bool cav = rowcav && in_cavity1(x, N);
         const double re = cav ? __ldg(srcc + x) : __ldg(src + x);
-        a[r] = make_double2(re, (finest || cav) ? 0.0 : re);
+        // rho_im (single-level plans only): a second, independent real field rides as the imaginary part —
+        // K-hat is real, so its potential comes out as the imaginary part of the result (cm_potential_modified)
+        a[r] = make_double2(re, rho_im ? __ldg(rho_im + row * N + x) : ((finest || cav) ? 0.0 : re));
     }
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
     {
@@ -226,13 +229,13 @@ __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const
 template <int T>
 __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ rho, const double *__restrict__ rc,
                                                     double2 *__restrict__ W1, const double2 *__restrict__ tw, int L,
-                                                    size_t row0)
+                                                    size_t row0, const double *__restrict__ rho_im)
 {
     // row0: first global row (b, z, y) of this launch
     constexpr int NN = 32 * T, ROWS = kThreads / T;
     extern __shared__ double2 smem[];
     const size_t row = row0 + (size_t)blockIdx.x * ROWS + threadIdx.x / T;
-    x_fwd_body<T>(rho, rc, W1 + row * NN, tw, L, row, smem);
+    x_fwd_body<T>(rho, rc, W1 + row * NN, tw, L, row, smem, rho_im);
 }
 
 // ====================== P5: x inverse + a8 (prolongation, Eq. 14) ==================
@@ -243,12 +246,13 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ r
 // p = N/4 + f/2 and sign s = +1 (f odd) / -1 (f even) gets
 //     ext_b(f) = 3/4 Hc[p] + 1/4 Hc[p+s]        (Eq. 3-6)
 //     Phi(Omega_b) = Phi^b + ext_b               (Eq. 14)
-// and hole_b = Phi_hole^b + ext_b is kept where the next level will read it.
+// and hole_b = Phi_hole^b + ext_b is kept where the next level will read it (on every cell if hole_all:
+// the modified method, Eq. B.1, builds Phi(Omega_b) from it).
 template <int T>
 __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
                                                     double *__restrict__ hole, const double *__restrict__ hole_c,
                                                     const double2 *__restrict__ tw, int L, double scale0 /* -G dx0^2 */,
-                                                    size_t row0)
+                                                    size_t row0, int hole_all, double *__restrict__ phi_im)
 {
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, Q = N / 4;
     using Lay = LayRow<T>;
@@ -296,7 +300,8 @@ __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ 
         const int x = j + T * r;
         const double re = scale * (e[r].x + o[r].x), im = scale * (e[r].y + o[r].y);
         dphi[x] = b > 0 ? re + ext[r] : re;
-        if (rowring && in_ring1(x, N)) dh[x] = b > 0 ? im + ext[r] : im;
+        if (hole_all ? (b < L - 1) : (rowring && in_ring1(x, N))) dh[x] = b > 0 ? im + ext[r] : im;
+        if (phi_im) phi_im[row * N + x] = im;       // the second field of a dual single-level solve
     }
 }
 
@@ -663,6 +668,46 @@ __global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, 
         zm = c;
         c = zp;
     }
+}
+
+// ============ f-2: modified ("dipole") method over neighbouring pairs, Eq. 15 / B.1-B.2 ============
+// dbl = the fine grid l1 expanded to the physical size of its parent (Fig. 14): (2N)^3 cells
+// of the fine size, the fine grid's density (finer levels projected onto it: rc) in the central N^3, zero around.
+__global__ void k_pad_dbl(int N, int l1, int L, const double *__restrict__ rho, const double *__restrict__ rc,
+                          double *__restrict__ dbl)
+{
+    const int n = 2 * N, h = N / 2, H = N / 2, Q = N / 4;
+    const size_t tot = (size_t)n * n * n, n3 = (size_t)N * N * N;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= tot) return;
+    const int i = (int)(idx % n) - h, j = (int)((idx / n) % n) - h, k = (int)(idx / ((size_t)n * n)) - h;
+    double v = 0.0;
+    if (i >= 0 && i < N && j >= 0 && j < N && k >= 0 && k < N) {
+        const bool cav = (l1 < L - 1) && in_cavity1(k, N) && in_cavity1(j, N) && in_cavity1(i, N);
+        v = cav ? rc[(size_t)l1 * (n3 / 8) + ((size_t)(k - Q) * H + (j - Q)) * H + (i - Q)]
+                : rho[(size_t)l1 * n3 + ((size_t)k * N + j) * N + i];
+    }
+    dbl[idx] = v;
+}
+
+// Phi(Omega_n) = [Phi_hole^n + ext_n] + scale * mean of the 8 doubled-grid cells under each coarse cell  (B.1)
+__global__ void k_combine_dbl(int N, const double *__restrict__ hole_n, const double *__restrict__ phi2, double scale,
+                              double *__restrict__ phi_n)
+{
+    const int n = 2 * N;
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)N * N * N) return;
+    const int i = (int)(idx % N), j = (int)((idx / N) % N), k = (int)(idx / ((size_t)N * N));
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            const double2 v = *reinterpret_cast<const double2 *>(phi2 + ((size_t)(2 * k + c) * n + (2 * j + b)) * n + 2 * i);
+            s += v.x;
+            s += v.y;
+        }
+    phi_n[idx] = hole_n[idx] + scale * (s / 8.0);
 }
 
 }  // namespace cmk

@@ -32,6 +32,11 @@ struct cm_plan {
     double *stage_rho = nullptr, *stage_phi = nullptr;
     size_t bytes = 0;
     bool green_ready = false;
+    int hole_all = 0;               // P5 keeps Phi_hole + ext on every cell (cm_potential_modified)
+    cm_plan *dbl = nullptr;         // single-level plan of the doubled fine grid (2N)^3, Eq. B.1
+    double *rho2 = nullptr, *phi2 = nullptr;   // two doubled grids each: one complex solve serves two pairs
+    const double *dual_in = nullptr;            // single-level plans: second real field in / its potential out
+    double *dual_out = nullptr;
     bool use_graph = true;
     cudaStream_t cap_stream = nullptr, copy_stream = nullptr;
     std::vector<cudaEvent_t> ev_level;   // cm_potential_host's pipeline: [0,32) level arrived, [32,64) level's Phi ready, [64] start
@@ -130,7 +135,7 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     }
     }
     if (!fused_done) {
-        k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
+        k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
         if (ev) cudaEventRecord(ev[2], s);
         if (T == 16) k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
         else k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
@@ -143,7 +148,7 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     const size_t lrows = (size_t)N * N;
     const unsigned gl = (unsigned)((lrows + ROWS - 1) / ROWS);
     for (int b = 0; b < L; ++b)
-        k_x_inv<T><<<gl, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, L, scale0, (size_t)b * lrows);
+        k_x_inv<T><<<gl, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, L, scale0, (size_t)b * lrows, p->hole_all, p->dual_out);
     if (ev) cudaEventRecord(ev[6], s);
     p->launches += (p->fused_fwd ? 3 : 4) + L;
     CM_CUDA(p, cudaGetLastError());
@@ -158,7 +163,7 @@ template <int T> void level_p1_to_p4(cm_plan *p, const double *rho, cudaStream_t
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = 8 * (16 / T);
     const size_t lrows = (size_t)N * N;
     double2 *w1 = p->W1 + (size_t)l * lrows * NN, *w2 = p->W2 + (size_t)l * N * NN * NN;
-    k_x_fwd<T><<<(unsigned)(lrows / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows);
+    k_x_fwd<T><<<(unsigned)(lrows / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows, nullptr);
     k_y_fwd<T><<<(unsigned)((size_t)N * NN / PEN), kThreads, smem_batch<T>(), s>>>(w1, w2, p->tw);
     launch_zconv<T>(p, s, l, 1);
     k_y_inv<T><<<(unsigned)((size_t)N * NN / PEN), kThreads, smem_batch<T>(), s>>>(w2, w1, p->tw);
@@ -168,7 +173,7 @@ template <int T> void level_p5(cm_plan *p, double *phi, cudaStream_t s, int l)
     constexpr int N = 16 * T, ROWS = kThreads / T;
     const size_t lrows = (size_t)N * N;
     k_x_inv<T><<<(unsigned)((lrows + ROWS - 1) / ROWS), kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, p->L,
-                                                                                   -p->G * p->dx0 * p->dx0, (size_t)l * lrows);
+                                                                                   -p->G * p->dx0 * p->dx0, (size_t)l * lrows, p->hole_all, nullptr);
 }
 void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int l, bool p5)
 {
@@ -522,6 +527,54 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
     return CM_OK;
 }
 
+int cm_potential_modified(cm_plan *p, const double *rho, double *phi, void *stream)
+{
+    if (!p || !rho || !phi) return CM_EINVAL;
+    if (((uintptr_t)rho & 15) || ((uintptr_t)phi & 15)) return CM_EINVAL;
+    if (!p->green_ready) return CM_ENOTREADY;
+    if (p->N > 128) return CM_EINVAL;                      // the doubled grid must be a supported size
+    const size_t n3 = (size_t)p->N * p->N * p->N, tot = (size_t)p->L * n3;
+    if ((rho <= phi && phi < rho + tot) || (phi <= rho && rho < phi + tot)) return CM_EINVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (p->L > 1 && !p->dbl) {
+        int rc = cm_plan_create(&p->dbl, 2 * p->N, 1, 1.0, 2);
+        if (rc == CM_OK) rc = cm_green_precompute(p->dbl);
+        if (rc == CM_OK) rc = dev_alloc(p, &p->rho2, 2 * 8 * n3);
+        if (rc == CM_OK) rc = dev_alloc(p, &p->phi2, 2 * 8 * n3);
+        if (rc != CM_OK) {
+            if (p->dbl) std::snprintf(p->err, sizeof(p->err), "doubled-grid plan: %s", p->dbl->err);
+            return rc;
+        }
+        p->bytes += p->dbl->bytes;
+    }
+    // the original solve, keeping H_n = Phi_hole^n + ext_n on every cell; the finest level's Phi is final (B.2)
+    p->hole_all = 1;
+    int rc = enqueue_solve(p, rho, phi, s);
+    p->hole_all = 0;
+    if (rc != CM_OK) return rc;
+    // every pair n : n+1 (B.1); two pairs per doubled-grid solve: the second doubled density rides as the
+    // imaginary part of the complex field (K-hat is real), so its potential is the imaginary part of the result
+    const size_t d3 = 8 * n3;
+    for (int n = 0; n + 1 < p->L; n += 2) {
+        const bool two = n + 2 < p->L;
+        k_pad_dbl<<<(unsigned)((d3 + 255) / 256), 256, 0, s>>>(p->N, n + 1, p->L, rho, p->rc, p->rho2);
+        if (two) k_pad_dbl<<<(unsigned)((d3 + 255) / 256), 256, 0, s>>>(p->N, n + 2, p->L, rho, p->rc, p->rho2 + d3);
+        p->dbl->dual_in = two ? p->rho2 + d3 : nullptr;
+        p->dbl->dual_out = two ? p->phi2 + d3 : nullptr;
+        rc = enqueue_solve(p->dbl, p->rho2, p->phi2, s);   // plan of unit G and dx: phi2 = -(rho2 * g)
+        p->dbl->dual_in = nullptr;
+        p->dbl->dual_out = nullptr;
+        if (rc != CM_OK) return rc;
+        for (int q = 0; q < (two ? 2 : 1); ++q) {
+            const double dxf = p->dx0 * std::exp2(-(double)(n + q + 1));
+            k_combine_dbl<<<(unsigned)((n3 + 255) / 256), 256, 0, s>>>(p->N, p->hole + (n + q) * n3, p->phi2 + q * d3, p->G * dxf * dxf,
+                                                                    phi + (n + q) * n3);
+        }
+    }
+    CM_CUDA(p, cudaGetLastError());
+    return CM_OK;
+}
+
 int cm_acceleration(cm_plan *p, const double *phi, double *g, void *stream)
 {
     if (!p || !phi || !g) return CM_EINVAL;
@@ -557,6 +610,9 @@ int cm_plan_destroy(cm_plan *p)
     cudaFree(p->rc);
     cudaFree(p->hole);
     cudaFree(p->pbar);
+    cudaFree(p->rho2);
+    cudaFree(p->phi2);
+    if (p->dbl) cm_plan_destroy(p->dbl);
     cudaFree(p->ctl);
     cudaFree(p->tw);
     cudaFree(p->stage_rho);
