@@ -238,6 +238,40 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ r
     x_fwd_body<T>(rho, rc, W1 + row * NN, tw, L, row, smem, rho_im);
 }
 
+// P1 split by output parity (see k_y_fwd_split): 256 threads, warps 0-3 the even slots, warps 4-7 the odd ones
+// of the SAME rows.
+template <int T>
+__global__ void __launch_bounds__(2 * kThreads, 2) k_x_fwd_split(const double *__restrict__ rho, const double *__restrict__ rc,
+                                                                 double2 *__restrict__ W1, const double2 *__restrict__ tw, int L)
+{
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, H = N / 2, Q = N / 4;
+    using Lay = LayRow<T>;
+    extern __shared__ double2 smem[];
+    const int P = threadIdx.x / kThreads, tid = threadIdx.x % kThreads, j = tid % T, rowl = tid / T;
+    const size_t row = (size_t)blockIdx.x * ROWS + rowl;
+    const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
+    const bool finest = (b == L - 1);
+    const bool rowcav = !finest && in_cavity1(z, N) && in_cavity1(y, N);
+    const double *src = rho + row * N;
+    const double *srcc = rowcav ? rc + (((size_t)b * H + (z - Q)) * H + (y - Q)) * H - Q : rho;
+    double2 a[16], v[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) {
+        const int x = j + T * r;
+        const bool cav = rowcav && in_cavity1(x, N);
+        const double re = cav ? __ldg(srcc + x) : __ldg(src + x);
+        a[r] = make_double2(re, (finest || cav) ? 0.0 : re);
+    }
+    double2 *buf = smem + (P * ROWS + rowl) * Lay::PS;
+    if (P == 0) fwd_half<T, 0, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncWarp());
+    else fwd_half<T, 1, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncWarp());
+    double2 *dst = W1 + row * NN + P * N;
+#pragma unroll
+    for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+        for (int k2 = 0; k2 < T; ++k2) dst[16 * k2 + cc * T + j] = v[cc * T + k2];
+}
+
 // ====================== P5: x inverse + a8 (prolongation, Eq. 14) ==================
 // One launch per level b, coarse -> fine (row0 = b N^2): the level's rows are transformed back,
 // cropped to x < N and scaled by -G dx_b^2; then the contribution of the coarser levels is added
@@ -370,6 +404,40 @@ __global__ void __launch_bounds__(kThreads, 3) k_y_fwd_occ3(const double2 *__res
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
     y_fwd_body<T, false>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
+}
+
+// P2 split by output parity: 256 threads, warps 0-3 form the even slots (P = 0), warps 4-7 the odd ones
+// (P = 1) of the SAME columns.  The two halves of a forward transform share nothing but their input, so
+// each thread carries one half only: about half the registers, twice the warps per SM (latency hiding),
+// at the price of reading the input twice (the second read is an L1/L2 hit).
+struct SyncParity {
+    int id;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+};
+template <int T>
+__global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *__restrict__ W1, double2 *__restrict__ W2,
+                                                                 const double2 *__restrict__ tw)
+{
+    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    using Lay = LayBatch<T>;
+    extern __shared__ double2 smem[];
+    const int P = threadIdx.x / kThreads, tid = threadIdx.x % kThreads;
+    const int px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
+    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
+    const size_t bz = q / NN;
+    const int sx = (int)(q % NN);
+    const double2 *src = W1 + bz * N * NN + sx;
+    double2 *dst = W2 + bz * NN * NN + sx + (size_t)P * N * NN;
+    double2 *buf = smem + (P * PEN + g * 8 + px) * Lay::PS;
+    double2 a[16], v[16];
+#pragma unroll
+    for (int r = 0; r < 16; ++r) a[r] = src[(size_t)(j + T * r) * NN];
+    if (P == 0) fwd_half<T, 0, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncParity{1});
+    else fwd_half<T, 1, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncParity{2});
+#pragma unroll
+    for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+        for (int k2 = 0; k2 < T; ++k2) dst[(size_t)(16 * k2 + cc * T + j) * NN] = v[cc * T + k2];
 }
 
 // ================================ P4: y inverse ====================================

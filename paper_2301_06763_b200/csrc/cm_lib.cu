@@ -32,6 +32,7 @@ struct cm_plan {
     double *stage_rho = nullptr, *stage_phi = nullptr;
     size_t bytes = 0;
     bool green_ready = false;
+    bool split_x = false, split_y = false;   // P1 / P2 split by output parity (256-thread CTAs): default at N = 256
     int hole_all = 0;               // P5 keeps Phi_hole + ext on every cell (cm_potential_modified)
     cm_plan *dbl = nullptr;         // single-level plan of the doubled fine grid (2N)^3, Eq. B.1
     double *rho2 = nullptr, *phi2 = nullptr;   // two doubled grids each: one complex solve serves two pairs
@@ -44,7 +45,6 @@ struct cm_plan {
     int launches = 0;
     int num_sms = 148;
     int zconv_grid = 0;
-    int zconv_mode = 0;             // 2 = parity-split direct kernel
     bool zconv_tma = true;          // P3 through the TMA-fed persistent kernel (CM_ZCONV=direct selects the first version)
     CUtensorMap mapW, mapK;
     int kernels_per_solve = 0;
@@ -78,11 +78,11 @@ template <int T> int set_attrs(cm_plan *p)
     CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_occ3<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_ps<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)(sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T))));
     if constexpr (T >= 8)
         CM_CUDA(p, cudaFuncSetAttribute(k_xy_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>())));
@@ -96,13 +96,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
 {
     constexpr int N = 16 * T, NN = 2 * N;
     const unsigned gz = (unsigned)((size_t)NN * NN / (8 * (16 / T)) * L);
-    if (p->zconv_mode == 2) {
-        const size_t sm = sizeof(double2) * (2 * (8 * (16 / T)) * LayBatch<T>::PS + 32 * T);
-        const int ntile = NN * NN / (8 * (16 / T));
-        int lo = p->zconv_grid > 0 ? p->zconv_grid : 64;
-        while (ntile % lo) lo >>= 1;
-        k_z_conv_ps<T><<<gz, 256, sm, s>>>(p->W2, p->Khat, p->tw, L, lo);
-    } else if (p->zconv_tma) {
+    if (p->zconv_tma) {
         const int ngroups = NN * NN / ZConvCfg<T>::PEN;
         // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
         const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
@@ -135,9 +129,11 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     }
     }
     if (!fused_done) {
-        k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
+        if (p->split_x && !p->dual_in) k_x_fwd_split<T><<<(unsigned)(planes * N / ROWS), 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
+        else k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
         if (ev) cudaEventRecord(ev[2], s);
-        if (T == 16) k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+        if (p->split_y) k_y_fwd_split<T><<<(unsigned)(planes * NN / PEN), 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+        else if (T == 16) k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
         else k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     }
     if (ev) cudaEventRecord(ev[3], s);
@@ -359,7 +355,10 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
     if (rc == CM_OK) {
         const char *zc = std::getenv("CM_ZCONV");
         p->zconv_tma = !(zc && std::strcmp(zc, "direct") == 0);
-        if (zc && std::strcmp(zc, "ps") == 0) p->zconv_mode = 2;
+        const char *sy = std::getenv("CM_SPLIT_Y");
+        p->split_y = sy ? sy[0] == '1' : (N == 256);   // measured: -5 % at N = 256, neutral or worse below
+        const char *sxe = std::getenv("CM_SPLIT_X");
+        p->split_x = sxe ? sxe[0] == '1' : (N == 256);   // measured: -14 % at N = 256, +6 % at N = 128
         const char *zg = std::getenv("CM_ZCONV_GRID");
         p->zconv_grid = zg ? std::atoi(zg) : 0;
         int dev = 0;
@@ -478,7 +477,7 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
         if (rc != CM_OK) return rc;
     }
     cudaStream_t s = (cudaStream_t)stream;
-    if (p->N < 128 || !p->zconv_tma || p->zconv_mode == 2) {
+    if (p->N < 128 || !p->zconv_tma) {
         // small grids are launch-bound, not link-bound: one copy in, the graph, one copy out
         CM_CUDA(p, cudaMemcpyAsync(p->stage_rho, rho_host, tot * sizeof(double), cudaMemcpyHostToDevice, s));
         const int rc = cm_potential(p, p->stage_rho, p->stage_phi, stream);

@@ -259,96 +259,4 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
 }
 
 
-// ====================== P3, parity-split variant (no TMA) ==========================
-// 256 threads: warps 0-3 take the even output frequencies (P = 0), warps 4-7 the odd ones
-// (P = 1) of the SAME 8*G pencils.  Each thread carries one parity only, which halves the
-// live registers (<= 128 -> 16 warps per SM instead of 8) and the serial work per thread;
-// the two partial inverse transforms are summed through shared memory at the end.
-struct NamedBar {
-    int id;
-    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
-};
-
-template <int T, int P>
-__device__ __forceinline__ void zconv_ps_half(const double2 (&a)[16], const double (&kk)[16], double2 (&o)[16], int j,
-                                              double2 *buf, const TwShared<T> &tws)
-{
-    using Lay = LayBatch<T>;
-    double2 v[16];
-    fwd_half<T, P, Lay, false>(a, v, j, buf, tws, NamedBar{1 + P});
-#pragma unroll
-    for (int i = 0; i < 16; ++i) {
-        v[i].x *= kk[i];
-        v[i].y *= kk[i];
-    }
-    inv_half<T, P, Lay, true>(v, o, j, buf, tws, NamedBar{1 + P});
-}
-
-template <int T>
-__global__ void __launch_bounds__(256, 2) k_z_conv_ps(double2 *__restrict__ W2, const double *__restrict__ Khat,
-                                                      const double2 *__restrict__ tw, int L, int lo_tiles)
-{
-    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
-    using Lay = LayBatch<T>;
-    extern __shared__ double2 smem[];
-    double2 *tw_s = smem + 2 * PEN * Lay::PS;
-    const int P = threadIdx.x >> 7, t = threadIdx.x & 127, px = t & 7, j = (t >> 3) % T, g = t / (8 * T);
-    // block order: [tile_hi][b][tile_lo], tile_lo < lo_tiles: lo_tiles adjacent tiles of one level run
-    // together (contiguous lo_tiles*PEN*16 bytes per z row -> DRAM page locality), and their K-hat
-    // tiles (lo_tiles * 32 KB) stay in L2 across the L levels.
-    const int chunk = lo_tiles * L;
-    const int hi = blockIdx.x / chunk, rem = blockIdx.x - hi * chunk;
-    const int b = rem / lo_tiles, tile = hi * lo_tiles + (rem - b * lo_tiles);
-    const size_t flat = (size_t)tile * PEN + g * 8 + px;   // sy * 2N + sx
-    const size_t zs = (size_t)NN * NN;
-    double2 *base = W2 + (size_t)b * N * zs + flat;
-    const double *kh = Khat + flat + (size_t)P * N * zs;
-    double2 *buf = smem + (P * PEN + g * 8 + px) * Lay::PS;
-    double2 *buf1 = smem + (PEN + g * 8 + px) * Lay::PS;               // the odd group's buffer
-
-    double2 a[16];
-    double kk[16];
-#ifndef ABL_NOGLOBAL
-#pragma unroll
-    for (int r = 0; r < 16; ++r) a[r] = base[(size_t)(j + T * r) * zs];
-#pragma unroll
-    for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-        for (int k2 = 0; k2 < T; ++k2) kk[cc * T + k2] = __ldg(kh + (size_t)(16 * k2 + cc * T + j) * zs);
-#else
-#pragma unroll
-    for (int r = 0; r < 16; ++r) { a[r] = make_double2(threadIdx.x + r, blockIdx.x - r); kk[r] = 0.5 + r; }
-#endif
-    for (int i = threadIdx.x; i < 32 * T; i += 256) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
-    __syncthreads();
-    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j]};
-
-    double2 o[16];
-#ifdef ABL_NOCOMPUTE
-    if (P == 0) {
-#pragma unroll
-        for (int r = 0; r < 16; ++r) base[(size_t)(j + T * r) * zs] = make_double2(a[r].x * kk[r], a[r].y);
-    }
-    return;
-#endif
-    if (P == 0) {
-        zconv_ps_half<T, 0>(a, kk, o, j, buf, tws);
-        __syncthreads();                       // the odd half's partial result is in buf1
-#pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            const double2 res = cadd(o[r], buf1[r * T + j]);
-#ifdef ABL_NOGLOBAL
-            if (res.x == 1.2345e-300)
-#endif
-            base[(size_t)(j + T * r) * zs] = res;
-        }
-    } else {
-        zconv_ps_half<T, 1>(a, kk, o, j, buf, tws);
-        NamedBar{2}();                         // every odd-group thread is done reading the exchange buffer
-#pragma unroll
-        for (int r = 0; r < 16; ++r) buf[r * T + j] = o[r];
-        __syncthreads();
-    }
-}
-
 }  // namespace cmk
