@@ -137,6 +137,17 @@ int cm_acceleration(cm_plan *plan, const double *phi_levels, double *g_levels, v
  */
 int cm_potential_modified(cm_plan *plan, const double *rho_levels, double *phi_levels, void *stream);
 
+/*
+ * Direct fine -> coarse summation (Eq. B.7): the input of grid `src_level`
+ * to the potential on the coarser grid `dst_level`,
+ *     Phi_ds(t) = -G sum_s rho_s dx_src^3 / |r_t - r_s|        (cell centres; all N^3 cells s of the source grid),
+ * the paper's substitute for the quadrupled grid of the triplet scheme when N <= 32 (L461).  O(N^6) work.
+ *   rho_levels : device, const, [levels][N][N][N]; only level src_level is read, as given (no projection).
+ *   phi_dst    : device, [N][N][N] fp64, overwritten with Phi_ds on every cell of level dst_level.
+ * 0 <= dst_level < src_level < levels, else CM_EINVAL.  Enqueues one kernel on `stream`.
+ */
+int cm_direct_sum(cm_plan *plan, const double *rho_levels, int src_level, int dst_level, double *phi_dst, void *stream);
+
 /* Release the plan and everything it owns.  NULL is accepted. */
 int cm_plan_destroy(cm_plan *plan);
 

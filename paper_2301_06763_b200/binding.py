@@ -17,7 +17,7 @@ CM_OK, CM_EINVAL, CM_ENOMEM, CM_ECUDA, CM_ENOTREADY = 0, -1, -2, -3, -4
 CM_BUF_RESTRICTED, CM_BUF_HOLE, CM_BUF_KHAT = 0, 1, 2
 
 EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potential_host", "cm_potential_profile",
-           "cm_acceleration", "cm_potential_modified",
+           "cm_acceleration", "cm_potential_modified", "cm_direct_sum",
            "cm_plan_destroy",
            "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
            "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error"]
@@ -43,6 +43,7 @@ def lib() -> C.CDLL:
     L.cm_potential_profile.argtypes = [vp, vp, vp, vp, C.POINTER(C.c_float), C.c_int]
     L.cm_acceleration.argtypes = [vp, vp, vp, vp]
     L.cm_potential_modified.argtypes = [vp, vp, vp, vp]
+    L.cm_direct_sum.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
     L.cm_plan_destroy.argtypes = [vp]
     L.cm_plan_set_G.argtypes = [vp, C.c_double]
     L.cm_plan_workspace_bytes.argtypes = [vp]
@@ -94,6 +95,10 @@ def cm_potential_profile(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0)
 
 def cm_potential_modified(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0) -> None:
     _check(lib().cm_potential_modified(plan, rho_ptr, phi_ptr, stream), plan)
+
+
+def cm_direct_sum(plan: int, rho_ptr: int, src_level: int, dst_level: int, phi_ptr: int, stream: int = 0) -> None:
+    _check(lib().cm_direct_sum(plan, rho_ptr, int(src_level), int(dst_level), phi_ptr, stream), plan)
 
 
 def cm_acceleration(plan: int, phi_ptr: int, g_ptr: int, stream: int = 0) -> None:
@@ -165,6 +170,15 @@ class Plan:
         s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
         cm_potential_modified(self._h, rho.data_ptr(), phi.data_ptr(), s)
         return phi
+
+    def direct_sum(self, rho, src_level: int, dst_level: int, stream=None):
+        """Eq. B.7: potential of level src_level's mass on the cells of level dst_level, [N, N, N]."""
+        import torch
+        self._check_tensor(rho, "cuda")
+        out = torch.empty((self.N, self.N, self.N), dtype=torch.float64, device=rho.device)
+        s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
+        cm_direct_sum(self._h, rho.data_ptr(), src_level, dst_level, out.data_ptr(), s)
+        return out
 
     def acceleration(self, phi, g=None, stream=None):
         """g[levels, 3, N, N, N] = -grad phi (cm_acceleration)."""

@@ -778,4 +778,51 @@ __global__ void k_combine_dbl(int N, const double *__restrict__ hole_n, const do
     phi_n[idx] = hole_n[idx] + scale * (s / 8.0);
 }
 
+// ================= f-3: direct fine -> coarse summation, Eq. B.7 =================
+// Phi_ds(t) = -G sum_s M_s / |r_t - r_s| over all N^3 cells s of the source (finer) grid, for every cell t of
+// the coarser target grid; M_s = rho_s dx_s^3, distances between cell centres (never zero: a coarse centre is a
+// corner of fine cells).  One thread per target, the sources stream through shared memory as (x, y, z, M)
+// in tiles of 256.  fp64 ALU-bound: N^6 inverse square roots; the paper uses it for N <= 32 only.
+// gridDim.y source chunks (so that small grids still fill the GPU): chunk c sums sources [c, c+1) * n3 / gridDim.y
+// into part[c][t]; k_direct_reduce adds the chunks in a fixed order (deterministic).
+__global__ void __launch_bounds__(256) k_direct_sum(int N, double dxs, double dxd, const double *__restrict__ rho_src,
+                                                    double *__restrict__ part)
+{
+    __shared__ double4 src[256];
+    const size_t n3 = (size_t)N * N * N;
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int ti = (int)(t % N), tj = (int)((t / N) % N), tk = (int)((t / ((size_t)N * N)) % N);
+    const double half = 0.5 - 0.5 * N;
+    const double tx = (ti + half) * dxd, ty = (tj + half) * dxd, tz = (tk + half) * dxd;
+    const double m3 = dxs * dxs * dxs;
+    double acc = 0.0;
+    const size_t s_lo = n3 * blockIdx.y / gridDim.y, s_hi = n3 * (blockIdx.y + 1) / gridDim.y;
+    for (size_t base = s_lo; base < s_hi; base += 256) {
+        const size_t s = base + threadIdx.x;
+        if (s < s_hi) {
+            const int si = (int)(s % N), sj = (int)((s / N) % N), sk = (int)(s / ((size_t)N * N));
+            src[threadIdx.x] = make_double4((si + half) * dxs, (sj + half) * dxs, (sk + half) * dxs, rho_src[s] * m3);
+        } else {
+            src[threadIdx.x] = make_double4(0.0, 0.0, 0.0, 0.0);   // zero mass at the origin: distance > 0 for every target
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int q = 0; q < 256; ++q) {
+            const double4 v = src[q];
+            const double ex = tx - v.x, ey = ty - v.y, ez = tz - v.z;
+            acc += v.w / sqrt(ex * ex + ey * ey + ez * ez);
+        }
+        __syncthreads();
+    }
+    if (t < n3) part[(size_t)blockIdx.y * n3 + t] = acc;
+}
+__global__ void k_direct_reduce(size_t n3, int chunks, double G, const double *__restrict__ part, double *__restrict__ phi_dst)
+{
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n3) return;
+    double acc = 0.0;
+    for (int c = 0; c < chunks; ++c) acc += part[(size_t)c * n3 + t];
+    phi_dst[t] = -G * acc;
+}
+
 }  // namespace cmk

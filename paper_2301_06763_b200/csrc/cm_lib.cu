@@ -574,6 +574,26 @@ int cm_potential_modified(cm_plan *p, const double *rho, double *phi, void *stre
     return CM_OK;
 }
 
+int cm_direct_sum(cm_plan *p, const double *rho_levels, int src_level, int dst_level, double *phi_dst, void *stream)
+{
+    if (!p || !rho_levels || !phi_dst) return CM_EINVAL;
+    if (dst_level < 0 || src_level <= dst_level || src_level >= p->L) return CM_EINVAL;
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    const double dxs = p->dx0 * std::exp2(-(double)src_level), dxd = p->dx0 * std::exp2(-(double)dst_level);
+    // enough source chunks for ~8 CTAs per SM; the partial sums live in W1 (free outside a solve: 4 N^3 doubles per level)
+    const unsigned tb = (unsigned)((n3 + 255) / 256);
+    int chunks = (8 * p->num_sms + (int)tb - 1) / (int)tb;
+    if (chunks < 1) chunks = 1;
+    if (chunks > 16) chunks = 16;
+    if (chunks > 4 * p->L) chunks = 4 * p->L;          // W1 holds 4 L N^3 doubles
+    cudaStream_t s = (cudaStream_t)stream;
+    double *part = reinterpret_cast<double *>(p->W1);
+    k_direct_sum<<<dim3(tb, chunks), 256, 0, s>>>(p->N, dxs, dxd, rho_levels + (size_t)src_level * n3, part);
+    k_direct_reduce<<<tb, 256, 0, s>>>(n3, chunks, p->G, part, phi_dst);
+    CM_CUDA(p, cudaGetLastError());
+    return CM_OK;
+}
+
 int cm_acceleration(cm_plan *p, const double *phi, double *g, void *stream)
 {
     if (!p || !phi || !g) return CM_EINVAL;
