@@ -11,10 +11,10 @@ from .cm_oracle import (build, lib, I0, restrict, field_direct, field_fft, green
                         fft1d, dft_naive, field_direct_at)
 
 from .cm_accel import acceleration, ghost_value, child_mean, padded_level
-from .cm_modified import solve_modified, doubled_density
+from .cm_modified import solve_modified, doubled_density, solve_modified_triplets, expanded_density, block_mean
 from .cm_direct import direct_sum
 
-__all__ = ["acceleration", "ghost_value", "child_mean", "padded_level", "solve_modified", "doubled_density", "direct_sum",
+__all__ = ["acceleration", "ghost_value", "child_mean", "padded_level", "solve_modified", "doubled_density", "solve_modified_triplets", "expanded_density", "block_mean", "direct_sum",
            "build", "lib", "I0", "restrict", "field_direct", "field_fft", "green_hat",
            "prolong", "solve", "solve_points", "leaf_direct", "num_threads",
            "fft1d", "dft_naive", "field_direct_at"]

@@ -37,6 +37,64 @@ def doubled_density(rhobar_fine: np.ndarray) -> np.ndarray:
     return out
 
 
+def expanded_density(rhobar_fine: np.ndarray, factor: int, hole: bool = False) -> np.ndarray:
+    """(factor N)^3 array at the fine cell size, concentric with the fine grid: the fine grid's density in the
+    central N^3 cells (with its own cavity [N/4, 3N/4)^3 zeroed if `hole`: the doubled grid "with a central hole"
+    of the triplet scheme, L448), zero in the added layers.  factor 2 = Omega_dbl, 4 = Omega_qdp (Fig. B.1)."""
+    N = rhobar_fine.shape[0]
+    core = np.array(rhobar_fine, dtype=np.float64, copy=True)
+    if hole:
+        q = N // 4
+        core[q:3 * q, q:3 * q, q:3 * q] = 0.0
+    out = np.zeros((factor * N,) * 3)
+    h = (factor - 1) * N // 2
+    out[h:h + N, h:h + N, h:h + N] = core
+    return out
+
+
+def block_mean(a: np.ndarray, factor: int) -> np.ndarray:
+    """Arithmetic mean over the factor^3 fine-size cells that make up each coarse cell (reading M2)."""
+    n = a.shape[0] // factor
+    return a.reshape(n, factor, n, factor, n, factor).mean(axis=(1, 3, 5))
+
+
+def solve_modified_triplets(rho: np.ndarray, dx0: float, G: float = 1.0, qdp: str = "fft"):
+    """rho [L,N,N,N] -> Phi [L,N,N,N] by Eq. B.3-B.6 (dipole moments across three neighbouring grids):
+
+        Phi(Omega^n) = Phi_hole^n + tilde Phi_dbl,hole^{n+1} + tilde Phi_qdp^{n+2} + sum_{k<n} tilde Phi_hole^k   (B.3, n < M-1)
+        Phi(Omega^n) = Phi_hole^n + tilde Phi_dbl^{n+1} + sum_{k<n} tilde Phi_hole^k                            (B.5, n = M-1)
+        Phi(Omega^n) = Phi^n + sum_{k<n} tilde Phi_hole^k                                                       (B.6, n = M)
+
+    qdp = "fft": the quadrupled grid (4N)^3 of Fig. B.1 by the same convolution, reduced by the mean over the 4^3
+    fine-size cells of a coarse cell; qdp = "direct": Eq. B.7 instead (cm_direct.direct_sum)."""
+    from .cm_direct import direct_sum
+    rho = np.ascontiguousarray(rho, dtype=np.float64)
+    L, N = rho.shape[0], rho.shape[1]
+    rhobar = restrict(rho)
+    gh = {1: green_hat(N)}
+    phi = np.empty_like(rho)
+    ext = np.zeros((N, N, N))
+    for l in range(L):
+        dx = dx0 / (1 << l)
+        if l == L - 1:
+            phi[l] = field_fft(rhobar[l], False, G, dx, gh[1]) + ext                                    # B.6
+            continue
+        hole = field_fft(rhobar[l], True, G, dx, gh[1])
+        gh.setdefault(2, green_hat(2 * N))
+        triple = l < L - 2
+        dbl = field_fft(expanded_density(rhobar[l + 1], 2, hole=triple), False, G, dx / 2, gh[2])
+        phi[l] = hole + block_mean(dbl, 2) + ext                                                        # B.5 / first terms of B.3
+        if triple:
+            if qdp == "fft":
+                gh.setdefault(4, green_hat(4 * N))
+                q = field_fft(expanded_density(rhobar[l + 2], 4), False, G, dx / 4, gh[4])
+                phi[l] = phi[l] + block_mean(q, 4)
+            else:
+                phi[l] = phi[l] + direct_sum(rhobar[l + 2], dx0, l + 2, l, G=G)                         # B.7
+        ext = prolong(ext + hole)
+    return phi
+
+
 def solve_modified(rho: np.ndarray, dx0: float, G: float = 1.0, method: str = "fft", return_parts: bool = False):
     """rho [L,N,N,N] -> Phi [L,N,N,N] by Eq. B.1-B.2 (pairs of neighbouring grids)."""
     rho = np.ascontiguousarray(rho, dtype=np.float64)

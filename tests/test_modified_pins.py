@@ -113,3 +113,81 @@ def test_appendix_c_ellipsoid_soft_pin():
     a, b = oracle.solve(rho, 4.5 / N), oracle.solve_modified(rho, 4.5 / N)
     d = 100 * np.abs((b - a) / a).max()
     assert bound / 4 < d < bound * 1.6
+
+
+# ------------------------------------------------------------------ triplet scheme, Eq. B.3-B.6
+def _exact_on_level0_from_level2(N, dx0, sources, G=1.0):
+    """Child-of-child mean (4^3 fine-size sub-cells per coarse cell) of the exact potential of level-2 point cells."""
+    dxf = dx0 / 4
+    sub = (np.arange(4 * N) + 0.5 - 2 * N) * dxf
+    Z, Y, X = np.meshgrid(sub, sub, sub, indexing="ij")
+    out = np.zeros_like(X)
+    for (k, j, i), rho_s in sources:
+        c = [(v + 0.5 - N / 2) * dxf for v in (k, j, i)]
+        d = np.sqrt((Z - c[0]) ** 2 + (Y - c[1]) ** 2 + (X - c[2]) ** 2)
+        with np.errstate(divide="ignore"):
+            out += np.where(d > 1e-12 * dx0, -G * rho_s * dxf ** 3 / d, -G * rho_s * dxf ** 2 * I0)
+    return oracle.block_mean(out, 4)
+
+
+def test_triplets_point_mass_two_levels_down_is_exact():
+    """B.3: a single cell of grid n+2 reaches grid n through the quadrupled grid: exactly the mean over the 64
+    fine-size sub-cells of the point-mass potential, on every cell of grid n."""
+    N, L, dx0 = 16, 3, 0.125
+    rho = np.zeros((L, N, N, N))
+    rho[2][5, 9, 6] = 3.0
+    phi = oracle.solve_modified_triplets(rho, dx0, G=1.3)
+    ref = _exact_on_level0_from_level2(N, dx0, [((5, 9, 6), 3.0)], G=1.3)
+    assert np.abs(phi[0] - ref).max() <= 1e-13 * np.abs(ref).max()
+
+
+def test_triplets_keep_a_dipole_that_the_pair_scheme_loses_two_levels_up():
+    """+q, -q in two children of one cell of grid 2 cancel when projected onto grid 1, so the pair scheme (whose
+    doubled grid carries grid 1's projected density) gives nothing on grid 0; the triplet scheme gives the exact
+    dipole potential there.  Grids 1 and 2 are the same in both schemes (B.5, B.6)."""
+    N, L, dx0 = 16, 3, 0.125
+    rho = np.zeros((L, N, N, N))
+    rho[2][8, 8, 8], rho[2][8, 8, 9] = 1.0, -1.0
+    pairs = oracle.solve_modified(rho, dx0)
+    trip = oracle.solve_modified_triplets(rho, dx0)
+    assert np.abs(pairs[0]).max() == 0.0
+    ref = _exact_on_level0_from_level2(N, dx0, [((8, 8, 8), 1.0), ((8, 8, 9), -1.0)])
+    assert np.abs(ref).max() > 0 and np.abs(trip[0] - ref).max() <= 1e-13 * np.abs(ref).max()
+    assert np.array_equal(trip[1], pairs[1]) and np.array_equal(trip[2], pairs[2])
+
+
+def test_triplets_do_not_count_mass_twice():
+    """The doubled grid of B.3 has a central hole exactly where grid n+2 lives (L448).  Far field: the total mass
+    seen from the corner of grid 0 is the same in the original, pair and triplet schemes."""
+    rng = np.random.default_rng(11)
+    N, L, dx0 = 16, 3, 0.125
+    rho = rng.random((L, N, N, N))
+    a, b, c = oracle.solve(rho, dx0), oracle.solve_modified(rho, dx0), oracle.solve_modified_triplets(rho, dx0)
+    assert abs(c[0][0, 0, 0] / a[0][0, 0, 0] - 1) < 1e-3 and abs(c[0][0, 0, 0] / b[0][0, 0, 0] - 1) < 1e-3
+    assert np.abs(c[0] / b[0] - 1).max() < 0.05
+
+
+def test_triplets_direct_summation_agrees_away_from_the_source_grid():
+    """B.7 in place of the quadrupled grid: centre sampling instead of the cell mean — the same to O(dx^2) away
+    from grid n+2 (which occupies the central quarter of grid n)."""
+    rng = np.random.default_rng(12)
+    N, L, dx0 = 16, 3, 0.125
+    rho = rng.random((L, N, N, N))
+    f = oracle.solve_modified_triplets(rho, dx0, qdp="fft")
+    d = oracle.solve_modified_triplets(rho, dx0, qdp="direct")
+    far = np.ones((N, N, N), bool)
+    far[4:12, 4:12, 4:12] = False
+    assert np.abs(d[0][far] / f[0][far] - 1).max() < 5e-3
+    assert np.array_equal(d[1], f[1]) and np.array_equal(d[2], f[2])
+
+
+def test_expanded_density_and_block_mean():
+    f = np.arange(8 ** 3, dtype=float).reshape(8, 8, 8) + 1
+    q = oracle.expanded_density(f, 4)
+    assert q.shape == (32, 32, 32) and q.sum() == f.sum() and np.array_equal(q[12:20, 12:20, 12:20], f)
+    h = oracle.expanded_density(f, 2, hole=True)
+    assert h.shape == (16, 16, 16) and h[4 + 2:4 + 6, 4 + 2:4 + 6, 4 + 2:4 + 6].sum() == 0
+    assert h.sum() == f.sum() - f[2:6, 2:6, 2:6].sum()
+    assert np.array_equal(oracle.expanded_density(f, 2), oracle.doubled_density(f))
+    m = oracle.block_mean(q, 4)
+    assert m.shape == (8, 8, 8) and abs(m[3, 3, 3] - q[12:16, 12:16, 12:16].mean()) < 1e-12
