@@ -138,6 +138,20 @@ int cm_acceleration(cm_plan *plan, const double *phi_levels, double *g_levels, v
 int cm_potential_modified(cm_plan *plan, const double *rho_levels, double *phi_levels, void *stream);
 
 /*
+ * The modified method with the dipole moments carried across THREE neighbouring grids (PAPER.md:L437-L448,
+ * Eq. B.3-B.6, Fig. B.1):
+ *     Phi(Omega^n) = Phi_hole^n + reduce(Phi_dbl,hole^{n+1}) + reduce(Phi_qdp^{n+2}) + sum_{k<n} tilde Phi_hole^k   (n < M-1)
+ *     Phi(Omega^n) = Phi_hole^n + reduce(Phi_dbl^{n+1}) + sum_{k<n} tilde Phi_hole^k                              (n = M-1)
+ *     Phi(Omega^n) = Phi^n + sum_{k<n} tilde Phi_hole^k                                                           (n = M)
+ * The doubled grid of grid n+1 has a central hole where grid n+2 lives (its mass is not counted twice); the
+ * quadrupled grid is grid n+2 expanded to the size of grid n ((4N)^3 cells of its own size), reduced by the mean over
+ * the 4^3 cells of a coarse cell.  qdp_direct != 0 replaces the quadrupled grid by the direct summation of Eq. B.7
+ * (cm_direct_sum; centre sampling instead of the cell mean).  N <= 64 (N <= 128 with qdp_direct), else CM_EINVAL.
+ * Other arguments and conventions as cm_potential_modified.
+ */
+int cm_potential_modified_triplets(cm_plan *plan, const double *rho_levels, double *phi_levels, int qdp_direct, void *stream);
+
+/*
  * Direct fine -> coarse summation (Eq. B.7): the input of grid `src_level`
  * to the potential on the coarser grid `dst_level`,
  *     Phi_ds(t) = -G sum_s rho_s dx_src^3 / |r_t - r_s|        (cell centres; all N^3 cells s of the source grid),

@@ -17,7 +17,7 @@ CM_OK, CM_EINVAL, CM_ENOMEM, CM_ECUDA, CM_ENOTREADY = 0, -1, -2, -3, -4
 CM_BUF_RESTRICTED, CM_BUF_HOLE, CM_BUF_KHAT = 0, 1, 2
 
 EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potential_host", "cm_potential_profile",
-           "cm_acceleration", "cm_potential_modified", "cm_direct_sum",
+           "cm_acceleration", "cm_potential_modified", "cm_potential_modified_triplets", "cm_direct_sum",
            "cm_plan_destroy",
            "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
            "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error"]
@@ -44,6 +44,7 @@ def lib() -> C.CDLL:
     L.cm_acceleration.argtypes = [vp, vp, vp, vp]
     L.cm_potential_modified.argtypes = [vp, vp, vp, vp]
     L.cm_direct_sum.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
+    L.cm_potential_modified_triplets.argtypes = [vp, vp, vp, C.c_int, vp]
     L.cm_plan_destroy.argtypes = [vp]
     L.cm_plan_set_G.argtypes = [vp, C.c_double]
     L.cm_plan_workspace_bytes.argtypes = [vp]
@@ -95,6 +96,10 @@ def cm_potential_profile(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0)
 
 def cm_potential_modified(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0) -> None:
     _check(lib().cm_potential_modified(plan, rho_ptr, phi_ptr, stream), plan)
+
+
+def cm_potential_modified_triplets(plan: int, rho_ptr: int, phi_ptr: int, qdp_direct: int = 0, stream: int = 0) -> None:
+    _check(lib().cm_potential_modified_triplets(plan, rho_ptr, phi_ptr, int(qdp_direct), stream), plan)
 
 
 def cm_direct_sum(plan: int, rho_ptr: int, src_level: int, dst_level: int, phi_ptr: int, stream: int = 0) -> None:
@@ -169,6 +174,17 @@ class Plan:
         self._check_tensor(phi, "cuda")
         s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
         cm_potential_modified(self._h, rho.data_ptr(), phi.data_ptr(), s)
+        return phi
+
+    def potential_modified_triplets(self, rho, phi=None, qdp_direct: bool = False, stream=None):
+        """Modified method over three neighbouring grids, Eq. B.3-B.6 (cm_potential_modified_triplets)."""
+        import torch
+        self._check_tensor(rho, "cuda")
+        if phi is None:
+            phi = torch.empty_like(rho)
+        self._check_tensor(phi, "cuda")
+        s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
+        cm_potential_modified_triplets(self._h, rho.data_ptr(), phi.data_ptr(), int(bool(qdp_direct)), s)
         return phi
 
     def direct_sum(self, rho, src_level: int, dst_level: int, stream=None):

@@ -738,44 +738,41 @@ __global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, 
     }
 }
 
-// ============ f-2: modified ("dipole") method over neighbouring pairs, Eq. 15 / B.1-B.2 ============
-// dbl = the fine grid l1 expanded to the physical size of its parent (Fig. 14): (2N)^3 cells
-// of the fine size, the fine grid's density (finer levels projected onto it: rc) in the central N^3, zero around.
-__global__ void k_pad_dbl(int N, int l1, int L, const double *__restrict__ rho, const double *__restrict__ rc,
-                          double *__restrict__ dbl)
+// ============ f-2: modified ("dipole") method, Eq. 15 / B.1-B.2 (pairs) and B.3-B.6 (triplets) ============
+// out = the fine grid l1 expanded F times (Fig. 14: F = 2, the doubled grid; L448 Fig. B.1: F = 4, the
+// quadrupled grid; F = 1: the grid itself): (F N)^3 cells of the fine size, concentric; the fine grid's density
+// (finer levels projected onto it: rc) in the central N^3, zero around; `hole`: its own cavity zeroed as well
+// (the doubled grid "with a central hole" of the triplet scheme, so that grid l1+1's mass is not counted twice).
+__global__ void k_pad_expand(int N, int F, int hole, int l1, int L, const double *__restrict__ rho, const double *__restrict__ rc,
+                             double *__restrict__ out)
 {
-    const int n = 2 * N, h = N / 2, H = N / 2, Q = N / 4;
+    const int n = F * N, h = (F - 1) * N / 2, H = N / 2, Q = N / 4;
     const size_t tot = (size_t)n * n * n, n3 = (size_t)N * N * N;
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= tot) return;
     const int i = (int)(idx % n) - h, j = (int)((idx / n) % n) - h, k = (int)(idx / ((size_t)n * n)) - h;
     double v = 0.0;
     if (i >= 0 && i < N && j >= 0 && j < N && k >= 0 && k < N) {
-        const bool cav = (l1 < L - 1) && in_cavity1(k, N) && in_cavity1(j, N) && in_cavity1(i, N);
-        v = cav ? rc[(size_t)l1 * (n3 / 8) + ((size_t)(k - Q) * H + (j - Q)) * H + (i - Q)]
-                : rho[(size_t)l1 * n3 + ((size_t)k * N + j) * N + i];
+        const bool cav = in_cavity1(k, N) && in_cavity1(j, N) && in_cavity1(i, N);
+        if (!(cav && hole))
+            v = (cav && l1 < L - 1) ? rc[(size_t)l1 * (n3 / 8) + ((size_t)(k - Q) * H + (j - Q)) * H + (i - Q)]
+                                    : rho[(size_t)l1 * n3 + ((size_t)k * N + j) * N + i];
     }
-    dbl[idx] = v;
+    out[idx] = v;
 }
 
-// Phi(Omega_n) = [Phi_hole^n + ext_n] + scale * mean of the 8 doubled-grid cells under each coarse cell  (B.1)
-__global__ void k_combine_dbl(int N, const double *__restrict__ hole_n, const double *__restrict__ phi2, double scale,
-                              double *__restrict__ phi_n)
+// phi_n = base + scale * (mean of the F^3 cells of `big` ((F N)^3) under each cell)   (the "reduce" of B.1 / B.3)
+__global__ void k_add_block_mean(int N, int F, const double *base, const double *__restrict__ big, double scale, double *phi_n)
 {
-    const int n = 2 * N;
+    const int n = F * N;
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (size_t)N * N * N) return;
     const int i = (int)(idx % N), j = (int)((idx / N) % N), k = (int)(idx / ((size_t)N * N));
     double s = 0.0;
-#pragma unroll
-    for (int c = 0; c < 2; ++c)
-#pragma unroll
-        for (int b = 0; b < 2; ++b) {
-            const double2 v = *reinterpret_cast<const double2 *>(phi2 + ((size_t)(2 * k + c) * n + (2 * j + b)) * n + 2 * i);
-            s += v.x;
-            s += v.y;
-        }
-    phi_n[idx] = hole_n[idx] + scale * (s / 8.0);
+    for (int c = 0; c < F; ++c)
+        for (int b = 0; b < F; ++b)
+            for (int a = 0; a < F; ++a) s += big[((size_t)(F * k + c) * n + (F * j + b)) * n + F * i + a];
+    phi_n[idx] = base[idx] + scale * (s / (double)(F * F * F));
 }
 
 // ================= f-3: direct fine -> coarse summation, Eq. B.7 =================

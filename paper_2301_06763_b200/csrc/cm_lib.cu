@@ -34,7 +34,8 @@ struct cm_plan {
     bool green_ready = false;
     bool split_x = false, split_y = false;   // P1 / P2 split by output parity (256-thread CTAs): default at N = 256
     int hole_all = 0;               // P5 keeps Phi_hole + ext on every cell (cm_potential_modified)
-    cm_plan *dbl = nullptr;         // single-level plan of the doubled fine grid (2N)^3, Eq. B.1
+    cm_plan *dbl = nullptr, *qdp = nullptr;   // single-level plans of the doubled (2N)^3 and quadrupled (4N)^3 fine grid
+    double *rho4 = nullptr, *phi4 = nullptr, *tmp3 = nullptr;
     double *rho2 = nullptr, *phi2 = nullptr;   // two doubled grids each: one complex solve serves two pairs
     const double *dual_in = nullptr;            // single-level plans: second real field in / its potential out
     double *dual_out = nullptr;
@@ -526,58 +527,141 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
     return CM_OK;
 }
 
-int cm_potential_modified(cm_plan *p, const double *rho, double *phi, void *stream)
+}  // extern "C" (re-opened below)
+
+namespace {
+
+// one expanded-grid plan (N' = F N, one level, unit G and dx) with room for two fields (dual solve)
+int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **rho_big, double **phi_big)
 {
-    if (!p || !rho || !phi) return CM_EINVAL;
-    if (((uintptr_t)rho & 15) || ((uintptr_t)phi & 15)) return CM_EINVAL;
-    if (!p->green_ready) return CM_ENOTREADY;
-    if (p->N > 128) return CM_EINVAL;                      // the doubled grid must be a supported size
-    const size_t n3 = (size_t)p->N * p->N * p->N, tot = (size_t)p->L * n3;
-    if ((rho <= phi && phi < rho + tot) || (phi <= rho && rho < phi + tot)) return CM_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    if (p->L > 1 && !p->dbl) {
-        int rc = cm_plan_create(&p->dbl, 2 * p->N, 1, 1.0, 2);
-        if (rc == CM_OK) rc = cm_green_precompute(p->dbl);
-        if (rc == CM_OK) rc = dev_alloc(p, &p->rho2, 2 * 8 * n3);
-        if (rc == CM_OK) rc = dev_alloc(p, &p->phi2, 2 * 8 * n3);
-        if (rc != CM_OK) {
-            if (p->dbl) std::snprintf(p->err, sizeof(p->err), "doubled-grid plan: %s", p->dbl->err);
-            return rc;
-        }
-        p->bytes += p->dbl->bytes;
+    if (*plan) return CM_OK;
+    const size_t n3 = (size_t)p->N * p->N * p->N, big = (size_t)F * F * F * n3;
+    int rc = cm_plan_create(plan, F * p->N, 1, 1.0, 2);
+    if (rc == CM_OK) rc = cm_green_precompute(*plan);
+    if (rc == CM_OK) rc = dev_alloc(p, rho_big, 2 * big);
+    if (rc == CM_OK) rc = dev_alloc(p, phi_big, 2 * big);
+    if (rc != CM_OK) {
+        if (*plan) std::snprintf(p->err, sizeof(p->err), "expanded-grid plan (x%d): %s", F, (*plan)->err);
+        return rc;
     }
-    // the original solve, keeping H_n = Phi_hole^n + ext_n on every cell; the finest level's Phi is final (B.2)
+    p->bytes += (*plan)->bytes;
+    return CM_OK;
+}
+
+// Expanded grids of levels l1 and (optionally) l1b through ONE complex single-level solve (K-hat is real: the second
+// density rides as the imaginary part); results -(rho * g) in phi_big and phi_big + big.
+int solve_expanded(cm_plan *p, cm_plan *pe, int F, const double *rho, double *rho_big, double *phi_big, cudaStream_t s, int l1,
+                   int hole1, int l1b, int hole1b)
+{
+    const size_t n3 = (size_t)p->N * p->N * p->N, big = (size_t)F * F * F * n3;
+    const unsigned g = (unsigned)((big + 255) / 256);
+    k_pad_expand<<<g, 256, 0, s>>>(p->N, F, hole1, l1, p->L, rho, p->rc, rho_big);
+    if (l1b >= 0) k_pad_expand<<<g, 256, 0, s>>>(p->N, F, hole1b, l1b, p->L, rho, p->rc, rho_big + big);
+    pe->dual_in = l1b >= 0 ? rho_big + big : nullptr;
+    pe->dual_out = l1b >= 0 ? phi_big + big : nullptr;
+    const int rc = enqueue_solve(pe, rho_big, phi_big, s);
+    pe->dual_in = nullptr;
+    pe->dual_out = nullptr;
+    return rc;
+}
+
+int direct_sum_impl(cm_plan *p, const double *rho_src, int src_level, int dst_level, double *phi_dst, cudaStream_t s);
+
+// depth 2: Eq. B.1-B.2 (pairs); depth 3: Eq. B.3-B.6 (triplets), the quadrupled grid by FFT or by Eq. B.7
+int modified_impl(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int depth, int qdp_direct)
+{
+    const int N = p->N, L = p->L;
+    const size_t n3 = (size_t)N * N * N;
+    const unsigned gn = (unsigned)((n3 + 255) / 256);
+    int rc = CM_OK;
+    if (L > 1 && (rc = ensure_expanded(p, 2, &p->dbl, &p->rho2, &p->phi2)) != CM_OK) return rc;
+    const bool triple = depth == 3 && L > 2;
+    if (triple && !qdp_direct && (rc = ensure_expanded(p, 4, &p->qdp, &p->rho4, &p->phi4)) != CM_OK) return rc;
+    if (triple && qdp_direct && !p->tmp3 && (rc = dev_alloc(p, &p->tmp3, 2 * n3)) != CM_OK) return rc;
+    // the original solve, keeping H_n = Phi_hole^n + ext_n on every cell; the finest level's Phi is final (B.2 / B.6)
     p->hole_all = 1;
-    int rc = enqueue_solve(p, rho, phi, s);
+    rc = enqueue_solve(p, rho, phi, s);
     p->hole_all = 0;
     if (rc != CM_OK) return rc;
-    // every pair n : n+1 (B.1); two pairs per doubled-grid solve: the second doubled density rides as the
-    // imaginary part of the complex field (K-hat is real), so its potential is the imaginary part of the result
-    const size_t d3 = 8 * n3;
-    for (int n = 0; n + 1 < p->L; n += 2) {
-        const bool two = n + 2 < p->L;
-        k_pad_dbl<<<(unsigned)((d3 + 255) / 256), 256, 0, s>>>(p->N, n + 1, p->L, rho, p->rc, p->rho2);
-        if (two) k_pad_dbl<<<(unsigned)((d3 + 255) / 256), 256, 0, s>>>(p->N, n + 2, p->L, rho, p->rc, p->rho2 + d3);
-        p->dbl->dual_in = two ? p->rho2 + d3 : nullptr;
-        p->dbl->dual_out = two ? p->phi2 + d3 : nullptr;
-        rc = enqueue_solve(p->dbl, p->rho2, p->phi2, s);   // plan of unit G and dx: phi2 = -(rho2 * g)
-        p->dbl->dual_in = nullptr;
-        p->dbl->dual_out = nullptr;
+    // doubled grids: Phi(Omega^n) = H_n + reduce(Phi_dbl^{n+1}), two pairs per complex solve; in the triplet scheme the
+    // doubled grid has a central hole (grid n+2's mass comes through the quadrupled grid) except for the last pair (B.5)
+    const size_t d3 = 8 * n3, q3 = 64 * n3;
+    for (int n = 0; n + 1 < L; n += 2) {
+        const bool two = n + 2 < L;
+        const int h0 = triple && n < L - 2, h1 = triple && n + 1 < L - 2;
+        rc = solve_expanded(p, p->dbl, 2, rho, p->rho2, p->phi2, s, n + 1, h0, two ? n + 2 : -1, h1);
         if (rc != CM_OK) return rc;
         for (int q = 0; q < (two ? 2 : 1); ++q) {
             const double dxf = p->dx0 * std::exp2(-(double)(n + q + 1));
-            k_combine_dbl<<<(unsigned)((n3 + 255) / 256), 256, 0, s>>>(p->N, p->hole + (n + q) * n3, p->phi2 + q * d3, p->G * dxf * dxf,
-                                                                    phi + (n + q) * n3);
+            k_add_block_mean<<<gn, 256, 0, s>>>(N, 2, p->hole + (n + q) * n3, p->phi2 + q * d3, p->G * dxf * dxf, phi + (n + q) * n3);
+        }
+    }
+    // quadrupled grids (B.3): + reduce(Phi_qdp^{n+2}) for n < L-2, by the same convolution or by direct summation (B.7)
+    if (triple) {
+        for (int n = 0; n + 2 < L; n += (qdp_direct ? 1 : 2)) {
+            if (qdp_direct) {
+                k_pad_expand<<<gn, 256, 0, s>>>(N, 1, 0, n + 2, L, rho, p->rc, p->tmp3);           // rho-bar of grid n+2
+                rc = direct_sum_impl(p, p->tmp3, n + 2, n, p->tmp3 + n3, s);
+                if (rc != CM_OK) return rc;
+                k_add_block_mean<<<gn, 256, 0, s>>>(N, 1, phi + n * n3, p->tmp3 + n3, 1.0, phi + n * n3);
+            } else {
+                const bool two = n + 3 < L;
+                rc = solve_expanded(p, p->qdp, 4, rho, p->rho4, p->phi4, s, n + 2, 0, two ? n + 3 : -1, 0);
+                if (rc != CM_OK) return rc;
+                for (int q = 0; q < (two ? 2 : 1); ++q) {
+                    const double dxf = p->dx0 * std::exp2(-(double)(n + q + 2));
+                    k_add_block_mean<<<gn, 256, 0, s>>>(N, 4, phi + (n + q) * n3, p->phi4 + q * q3, p->G * dxf * dxf, phi + (n + q) * n3);
+                }
+            }
         }
     }
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
 
+int check_modified_args(cm_plan *p, const double *rho, double *phi)
+{
+    if (!p || !rho || !phi) return CM_EINVAL;
+    if (((uintptr_t)rho & 15) || ((uintptr_t)phi & 15)) return CM_EINVAL;
+    if (!p->green_ready) return CM_ENOTREADY;
+    const size_t tot = (size_t)p->L * p->N * p->N * p->N;
+    if ((rho <= phi && phi < rho + tot) || (phi <= rho && rho < phi + tot)) return CM_EINVAL;
+    return CM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int cm_potential_modified(cm_plan *p, const double *rho, double *phi, void *stream)
+{
+    const int rc = check_modified_args(p, rho, phi);
+    if (rc != CM_OK) return rc;
+    if (p->N > 128) return CM_EINVAL;                      // the doubled grid must be a supported size
+    return modified_impl(p, rho, phi, (cudaStream_t)stream, 2, 0);
+}
+
+int cm_potential_modified_triplets(cm_plan *p, const double *rho, double *phi, int qdp_direct, void *stream)
+{
+    const int rc = check_modified_args(p, rho, phi);
+    if (rc != CM_OK) return rc;
+    if (p->N > 128 || (!qdp_direct && p->N > 64)) return CM_EINVAL;   // 2N (and 4N) must be supported sizes
+    return modified_impl(p, rho, phi, (cudaStream_t)stream, 3, qdp_direct ? 1 : 0);
+}
+
 int cm_direct_sum(cm_plan *p, const double *rho_levels, int src_level, int dst_level, double *phi_dst, void *stream)
 {
     if (!p || !rho_levels || !phi_dst) return CM_EINVAL;
     if (dst_level < 0 || src_level <= dst_level || src_level >= p->L) return CM_EINVAL;
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    return direct_sum_impl(p, rho_levels + (size_t)src_level * n3, src_level, dst_level, phi_dst, (cudaStream_t)stream);
+}
+
+}  // extern "C"
+
+namespace {
+int direct_sum_impl(cm_plan *p, const double *rho_src, int src_level, int dst_level, double *phi_dst, cudaStream_t s)
+{
     const size_t n3 = (size_t)p->N * p->N * p->N;
     const double dxs = p->dx0 * std::exp2(-(double)src_level), dxd = p->dx0 * std::exp2(-(double)dst_level);
     // enough source chunks for ~8 CTAs per SM; the partial sums live in W1 (free outside a solve: 4 N^3 doubles per level)
@@ -586,13 +670,15 @@ int cm_direct_sum(cm_plan *p, const double *rho_levels, int src_level, int dst_l
     if (chunks < 1) chunks = 1;
     if (chunks > 16) chunks = 16;
     if (chunks > 4 * p->L) chunks = 4 * p->L;          // W1 holds 4 L N^3 doubles
-    cudaStream_t s = (cudaStream_t)stream;
     double *part = reinterpret_cast<double *>(p->W1);
-    k_direct_sum<<<dim3(tb, chunks), 256, 0, s>>>(p->N, dxs, dxd, rho_levels + (size_t)src_level * n3, part);
+    k_direct_sum<<<dim3(tb, chunks), 256, 0, s>>>(p->N, dxs, dxd, rho_src, part);
     k_direct_reduce<<<tb, 256, 0, s>>>(n3, chunks, p->G, part, phi_dst);
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
+}  // namespace
+
+extern "C" {
 
 int cm_acceleration(cm_plan *p, const double *phi, double *g, void *stream)
 {
@@ -632,6 +718,10 @@ int cm_plan_destroy(cm_plan *p)
     cudaFree(p->rho2);
     cudaFree(p->phi2);
     if (p->dbl) cm_plan_destroy(p->dbl);
+    if (p->qdp) cm_plan_destroy(p->qdp);
+    cudaFree(p->rho4);
+    cudaFree(p->phi4);
+    cudaFree(p->tmp3);
     cudaFree(p->ctl);
     cudaFree(p->tw);
     cudaFree(p->stage_rho);
