@@ -72,13 +72,16 @@ struct TwGlobal {
     static constexpr bool RECUR = false;
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return __ldg(&tw[j * (2 * k1 + P)]); }
     __device__ __forceinline__ double2 step() const { return make_double2(1.0, 0.0); }
+    __device__ __forceinline__ double2 step2() const { return make_double2(1.0, 0.0); }
+    __device__ __forceinline__ double2 step3() const { return make_double2(1.0, 0.0); }
 };
-// P3 is bound by the shared-memory data pipe (profiles/r01b), not by fp64: only the even-k1 twiddles are
-// read from the table; an odd one is the even one before it times rho = w_2N^{2j}, kept in registers
-// (one extra rounding, ~1e-16).
+// P3 is bound by the shared-memory data pipe (profiles/r01b), not by fp64: only every fourth twiddle (k1 = 0, 4,
+// 8, 12) is read from the table; the three after it are that one times rho, rho^2, rho^3 (rho = w_2N^{2j}, the
+// powers kept in registers; one extra rounding, ~1e-16).
 template <int T> struct TwShared {
     const double2 *base;   // table + j
     double2 rho;           // w_2N^{2 j}
+    double2 rho2, rho3;    // w_2N^{4 j}, w_2N^{6 j}
     static constexpr bool RECUR = true;
 #ifndef ABL_NOTW
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return base[(2 * k1 + P) * T]; }
@@ -86,12 +89,17 @@ template <int T> struct TwShared {
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return make_double2(0.6 + k1, 0.8 - P); }
 #endif
     __device__ __forceinline__ double2 step() const { return rho; }
+    __device__ __forceinline__ double2 step2() const { return rho2; }
+    __device__ __forceinline__ double2 step3() const { return rho3; }
 };
 
-// twiddle w_2N^{j (2 k1 + P)} for k1 = 0..15 in turn; `prev` carries the last even-k1 value
+// twiddle w_2N^{j (2 k1 + P)} for k1 = 0..15 in turn; `prev` carries the last value read from the table
 template <int P, class Tw> __device__ __forceinline__ double2 tw_next(const Tw &tw, int k1, double2 &prev)
 {
-    if (Tw::RECUR && (k1 & 1)) return (P == 0 && k1 == 1) ? tw.step() : cmul(prev, tw.step());
+    if (Tw::RECUR && (k1 & 3)) {
+        const double2 r = (k1 & 3) == 1 ? tw.step() : ((k1 & 3) == 2 ? tw.step2() : tw.step3());
+        return (P == 0 && k1 < 4) ? r : cmul(prev, r);
+    }
     prev = tw.template get<P>(k1);
     return prev;
 }
@@ -471,61 +479,6 @@ __global__ void __launch_bounds__(kThreads, T == 16 ? 3 : 2) k_y_inv(const doubl
     for (int r = 0; r < 16; ++r) dst[(size_t)(j + T * r) * NN] = cadd(e[r], o[r]);
 }
 
-// ====================== P3: z forward * K-hat * z inverse ==========================
-// blockIdx.x = tile * L + b: the L levels that share one K-hat tile run together so
-// the tile comes from HBM once and from L2 afterwards.
-template <int T>
-__global__ void __launch_bounds__(kThreads) k_z_conv(double2 *__restrict__ W2, const double *__restrict__ Khat,
-                                                     const double2 *__restrict__ tw, int L)
-{
-    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
-    using Lay = LayBatch<T>;
-    extern __shared__ double2 smem[];
-    const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
-    const int b = blockIdx.x % L;
-    const size_t flat = (size_t)(blockIdx.x / L) * PEN + g * 8 + px;   // sy * 2N + sx
-    const size_t zs = (size_t)NN * NN;
-    double2 *base = W2 + (size_t)b * N * zs + flat;
-    const double *kh = Khat + flat;
-    double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
-
-    double2 a[16];
-#pragma unroll
-    for (int r = 0; r < 16; ++r) a[r] = base[(size_t)(j + T * r) * zs];
-
-    double2 e[16];
-    {
-        double2 v[16];
-        fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncBlock());
-#pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-            for (int k2 = 0; k2 < T; ++k2) {
-                const double k = __ldg(kh + (size_t)(16 * k2 + cc * T + j) * zs);
-                v[cc * T + k2].x *= k;
-                v[cc * T + k2].y *= k;
-            }
-        inv_half<T, 0, Lay>(v, e, j, bufB, TwGlobal{tw, j}, SyncBlock());
-    }
-    {
-        double2 v[16], o[16];
-        fwd_half<T, 1, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncBlock());
-#pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-            for (int k2 = 0; k2 < T; ++k2) {
-                const double k = __ldg(kh + (size_t)(N + 16 * k2 + cc * T + j) * zs);
-                v[cc * T + k2].x *= k;
-                v[cc * T + k2].y *= k;
-            }
-        inv_half<T, 1, Lay>(v, o, j, bufB, TwGlobal{tw, j}, SyncBlock());
-#pragma unroll
-        for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
-    }
-#pragma unroll
-    for (int r = 0; r < 16; ++r) base[(size_t)(j + T * r) * zs] = e[r];
-}
-
 // ============================ a1: restriction cascade ==============================
 // rc[lf-1][ck][cj][ci] = mean of the 8 children of fine level lf, where a child that lies
 // under level lf+1 takes the already projected value rc[lf] (L280-L282; readings 9, 10).
@@ -596,16 +549,31 @@ __global__ void k_fft_simple(double2 *__restrict__ data, int n, int log2n, int a
     for (int i = threadIdx.x; i < n; i += blockDim.x) data[base + (size_t)i * stride] = sm[i];
 }
 
-// K-hat[sz][sy][sx] = Re Ghat[f(sz)][f(sy)][f(sx)] / (2N)^3, f = slot_to_freq.
-__global__ void k_green_permute(const double2 *__restrict__ Gm, double *__restrict__ Khat, int N)
+// Row stride (in doubles) of one pencil of K-hat: 2N slots + a pad that makes P3's shared-memory reads
+// conflict-free (a half-warp = T lanes j x 16/T pencils must hit 16 distinct 8-byte bank pairs: RSK = T mod 16).
+__host__ __device__ constexpr int khat_row_stride(int N) { return 2 * N + (N / 16 < 16 ? N / 16 : 0); }
+
+// K-hat, pencil-major: Kt[(sy 2N + sx) RSK + sz] = Re Ghat[f(sz)][f(sy)][f(sx)] / (2N)^3, f = slot_to_freq.  The PEN
+// pencils of one P3 tile are one contiguous block, fetched by a single bulk copy and read as it lies.
+__global__ void k_green_permute(const double2 *__restrict__ Gm, double *__restrict__ Kt, int N)
 {
-    const int n = 2 * N;
+    const int n = 2 * N, RSK = khat_row_stride(N);
     const size_t tot = (size_t)n * n * n;
     const double inv = 1.0 / ((double)n * (double)n * (double)n);
     for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < tot; q += (size_t)gridDim.x * blockDim.x) {
-        const int sx = (int)(q % n), sy = (int)((q / n) % n), sz = (int)(q / ((size_t)n * n));
+        const int sz = (int)(q % n), sx = (int)((q / n) % n), sy = (int)(q / ((size_t)n * n));
         const size_t fx = cmfft::slot_to_freq(sx, N), fy = cmfft::slot_to_freq(sy, N), fz = cmfft::slot_to_freq(sz, N);
-        Khat[q] = Gm[(fz * n + fy) * n + fx].x * inv;
+        Kt[((size_t)sy * n + sx) * RSK + sz] = Gm[(fz * n + fy) * n + fx].x * inv;
+    }
+}
+// test access: the same values as [sz][sy][sx]
+__global__ void k_khat_export(const double *__restrict__ Kt, double *__restrict__ out, int N)
+{
+    const int n = 2 * N, RSK = khat_row_stride(N);
+    const size_t tot = (size_t)n * n * n;
+    for (size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x; q < tot; q += (size_t)gridDim.x * blockDim.x) {
+        const int sx = (int)(q % n), sy = (int)((q / n) % n), sz = (int)(q / ((size_t)n * n));
+        out[q] = Kt[((size_t)sy * n + sx) * RSK + sz];
     }
 }
 

@@ -46,8 +46,7 @@ struct cm_plan {
     int launches = 0;
     int num_sms = 148;
     int zconv_grid = 0;
-    bool zconv_tma = true;          // P3 through the TMA-fed persistent kernel (CM_ZCONV=direct selects the first version)
-    CUtensorMap mapW, mapK;
+    CUtensorMap mapW;
     int kernels_per_solve = 0;
     bool fused_fwd = false;         // P1+P2 as one persistent kernel (cm_fused.cuh), N >= 128, CM_FUSE=1
     int fuse_R = 0, fuse_LAG = 0, fuse_grid = 0;
@@ -83,7 +82,6 @@ template <int T> int set_attrs(cm_plan *p)
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_occ3<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_z_conv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     if constexpr (T >= 8)
         CM_CUDA(p, cudaFuncSetAttribute(k_xy_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>())));
@@ -91,22 +89,16 @@ template <int T> int set_attrs(cm_plan *p)
     return CM_OK;
 }
 
-// P3 for every level in one launch (step a5).
-// levels [b0, b0 + L) of W2 (the TMA kernel only; the alternates take every level)
+// P3 (step a5) for levels [b0, b0 + L) of W2.
 template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
 {
     constexpr int N = 16 * T, NN = 2 * N;
-    const unsigned gz = (unsigned)((size_t)NN * NN / (8 * (16 / T)) * L);
-    if (p->zconv_tma) {
-        const int ngroups = NN * NN / ZConvCfg<T>::PEN;
-        // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
-        const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
-        int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
-        if (p->zconv_grid > 0 && p->zconv_grid < grid) grid = p->zconv_grid;
-        k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->mapK, p->W2, p->tw, L, ngroups, b0);
-    } else {
-        k_z_conv<T><<<gz, kThreads, smem_batch<T>(), s>>>(p->W2, p->Khat, p->tw, L);
-    }
+    const int ngroups = NN * NN / ZConvCfg<T>::PEN;
+    // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
+    const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
+    int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
+    if (p->zconv_grid > 0 && p->zconv_grid < grid) grid = p->zconv_grid;
+    k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0);
 }
 
 // The five FFT passes (steps a3-a7) with the prolongation + Eq. 14 sum (a8) folded into P5:
@@ -266,18 +258,6 @@ int make_tensor_maps(cm_plan *p)
             return CM_ECUDA;
         }
     }
-    {   // K-hat as fp64 [2N rows][(2N)^2]; box = 8 doubles (64 B) x min(2N, 256) rows, 64B swizzle
-        const cuuint64_t dims[2] = {NN * NN, NN};
-        const cuuint64_t strides[1] = {NN * NN * 8};
-        const cuuint32_t box[2] = {8, (cuuint32_t)(NN < 256 ? NN : 256)};
-        CUresult r = enc(&p->mapK, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->Khat, dims, strides, box, es,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        if (r != CUDA_SUCCESS) {
-            std::snprintf(p->err, sizeof(p->err), "cuTensorMapEncodeTiled(K-hat) failed: %d", (int)r);
-            return CM_ECUDA;
-        }
-    }
     return CM_OK;
 }
 
@@ -307,7 +287,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
     int rc = CM_OK;
     if ((rc = dev_alloc(p, &p->W1, L * N * N * n)) == CM_OK &&
         (rc = dev_alloc(p, &p->W2, L * N * n * n)) == CM_OK &&
-        (rc = dev_alloc(p, &p->Khat, n * n * n)) == CM_OK &&
+        (rc = dev_alloc(p, &p->Khat, n * n * (size_t)khat_row_stride(N))) == CM_OK &&
         (rc = dev_alloc(p, &p->rc, (L > 1 ? L - 1 : 1) * h3)) == CM_OK &&
         (rc = dev_alloc(p, &p->hole, L * n3)) == CM_OK &&
         (rc = dev_alloc(p, &p->pbar, (L > 1 ? L - 1 : 1) * h3)) == CM_OK &&
@@ -354,8 +334,6 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         p->ctl = (cmk::FusedCtl *)q;
     }
     if (rc == CM_OK) {
-        const char *zc = std::getenv("CM_ZCONV");
-        p->zconv_tma = !(zc && std::strcmp(zc, "direct") == 0);
         const char *sy = std::getenv("CM_SPLIT_Y");
         p->split_y = sy ? sy[0] == '1' : (N == 256);   // measured: -5 % at N = 256, neutral or worse below
         const char *sxe = std::getenv("CM_SPLIT_X");
@@ -366,7 +344,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         if (cuda_fail(p, cudaGetDevice(&dev), "cudaGetDevice") ||
             cuda_fail(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
             rc = CM_ECUDA;
-        else if (p->zconv_tma) rc = make_tensor_maps(p);
+        else rc = make_tensor_maps(p);
     }
     if (rc == CM_OK) {
         switch (p->T) {
@@ -478,7 +456,7 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
         if (rc != CM_OK) return rc;
     }
     cudaStream_t s = (cudaStream_t)stream;
-    if (p->N < 128 || !p->zconv_tma) {
+    if (p->N < 128) {
         // small grids are launch-bound, not link-bound: one copy in, the graph, one copy out
         CM_CUDA(p, cudaMemcpyAsync(p->stage_rho, rho_host, tot * sizeof(double), cudaMemcpyHostToDevice, s));
         const int rc = cm_potential(p, p->stage_rho, p->stage_phi, stream);
@@ -541,7 +519,7 @@ int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **rho_big, double 
     if (rc == CM_OK) rc = dev_alloc(p, rho_big, 2 * big);
     if (rc == CM_OK) rc = dev_alloc(p, phi_big, 2 * big);
     if (rc != CM_OK) {
-        if (*plan) std::snprintf(p->err, sizeof(p->err), "expanded-grid plan (x%d): %s", F, (*plan)->err);
+        if (*plan) std::snprintf(p->err, sizeof(p->err), "expanded-grid plan (x%d): %.400s", F, (*plan)->err);
         return rc;
     }
     p->bytes += (*plan)->bytes;
@@ -751,7 +729,11 @@ int cm_debug_copy(cm_plan *p, int which, double *dst, size_t n_doubles, void *st
     switch (which) {
         case CM_BUF_RESTRICTED: src = p->rc; cnt = (L - 1) * (n3 / 8); break;
         case CM_BUF_HOLE: src = p->hole; cnt = L * n3; break;
-        case CM_BUF_KHAT: src = p->Khat; cnt = 8 * n3; break;
+        case CM_BUF_KHAT:
+            if (n_doubles != 8 * n3) return CM_EINVAL;
+            k_khat_export<<<1024, 256, 0, (cudaStream_t)stream>>>(p->Khat, dst, p->N);
+            CM_CUDA(p, cudaGetLastError());
+            return CM_OK;
         default: return CM_EINVAL;
     }
     if (cnt != n_doubles) return CM_EINVAL;

@@ -11,7 +11,7 @@
 //   (the launch covers levels b0 .. b0 + L - 1: all of them in cm_potential, one in cm_potential_host's pipeline)
 //   * a CTA is persistent and walks tiles (g, b): g = a group of PEN adjacent (sy,sx)
 //     pencils, b = level.  All L levels of a group run back to back so the group's
-//     K-hat tile is fetched ONCE (TMA, 64B-swizzled) and stays in shared memory;
+//     K-hat tile is fetched ONCE (one bulk copy of its pencil-major block) and stays in shared memory;
 //   * the next tile's W2 data ([N z-rows][128 B], stride (2N)^2) is fetched by TMA
 //     (128B-swizzled box) while the current tile is being transformed; the tile is copied
 //     to registers as soon as it lands, which frees the stage for the following load;
@@ -77,9 +77,8 @@ template <int T> struct ZConvCfg {
     static constexpr int PEN = kThreads / T;          // pencils per tile
     static constexpr int NBOX = PEN / 8;              // 128-byte column groups per tile
     static constexpr int PPW = 32 / T;                // pencils per warp
-    static constexpr int KROWS = NN < 256 ? NN : 256; // rows of one K-hat TMA box (box dims <= 256)
-    static constexpr int KCH = NN / KROWS;
-    static constexpr uint32_t IN_BYTES = 32768, KH_BYTES = 32768;
+    static constexpr int RSK = khat_row_stride(N);    // doubles per pencil of the K-hat tile
+    static constexpr uint32_t IN_BYTES = 32768, KH_BYTES = PEN * RSK * 8;   // <= 33792, a multiple of 16
     // exchange buffer; at the end of a tile the same bytes stage the output tile for the TMA store
     static constexpr uint32_t EX_BYTES = (T > 1) ? PEN * LayRow<T>::PS * 16 : 32768;
     static_assert(EX_BYTES >= 32768, "the exchange buffer doubles as the 32 KB output stage");
@@ -91,11 +90,11 @@ template <int T> struct ZConvCfg {
 
 template <int T>
 __global__ void __launch_bounds__(kThreads, 2)
-k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ CUtensorMap mapK,
+k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict__ Kt,
              double2 *__restrict__ W2, const double2 *__restrict__ tw, int L, int ngroups, int b0)
 {
     using C = ZConvCfg<T>;
-    constexpr int N = C::N, NN = C::NN, PEN = C::PEN, NBOX = C::NBOX;
+    constexpr int N = C::N, PEN = C::PEN, NBOX = C::NBOX;
     using Lay = LayRow<T>;
     extern __shared__ unsigned char smem_raw[];
     const uint32_t s0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -145,11 +144,10 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
     auto issue_k = [&](int g) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         mbar_expect_tx(bar_k, C::KH_BYTES);
-#pragma unroll
-        for (int q = 0; q < NBOX; ++q)
-#pragma unroll
-            for (int c = 0; c < C::KCH; ++c)
-                tma_load_2d(s0 + C::OFF_KH + q * (NN * 64) + c * (C::KROWS * 64), &mapK, g * PEN + 8 * q, c * C::KROWS, bar_k);
+        // the PEN pencils of group g are one contiguous block of K-hat (pencil-major layout): one 1-D bulk copy
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(s0 + C::OFF_KH),
+                     "l"(Kt + (size_t)g * PEN * C::RSK), "r"(C::KH_BYTES), "r"(bar_k)
+                     : "memory");
     };
 
     if (tid == 0) {
@@ -167,12 +165,12 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
     }
 
     const unsigned char *in_p = sbase + C::OFF_IN + bx * (N * 128);
-    const unsigned char *kh_p = sbase + C::OFF_KH + bx * (NN * 64) + ((px & 1) << 3);
+    const double *kh_p = reinterpret_cast<const double *>(sbase + C::OFF_KH) + pen * C::RSK;
     double2 *ex_p = ex_s + pen * Lay::PS;
 #ifdef ZC_TWGLOBAL
     const TwGlobal tws{tw, j};
 #else
-    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j]};
+    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j], tw_s[4 * T + j], tw_s[6 * T + j]};
 #endif
 #ifdef ZC_SYNCBLOCK
     using SyncX = SyncBlock;
@@ -204,7 +202,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const __grid_constant__ C
 #pragma unroll
                 for (int k2 = 0; k2 < T; ++k2) {
                     const int s = P * N + 16 * k2 + cc * T + j;
-                    const double k = *reinterpret_cast<const double *>(kh_p + s * 64 + ((((px >> 1) ^ (s >> 1)) & 3) << 4));
+                    const double k = kh_p[s];
                     v[cc * T + k2].x *= k;
                     v[cc * T + k2].y *= k;
                 }
