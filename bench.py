@@ -399,15 +399,15 @@ def run_ours(args) -> None:
     }
     # P3 is bound on chip, not by HBM: fp64 instructions per thread-tile counted in the SASS of
     # k_z_conv_tma<T> (cuobjdump), peak = 64 fp64 lanes/clk/SM measured on this box (18.4 T lane-instr/s at 1965 MHz)
-    P3_FP64_PER_THREAD_TILE = {1: 796, 2: 1292, 4: 1420, 8: 1596, 16: 1788}
+    P3_FP64_PER_THREAD_TILE = {1: 796, 2: 1340, 4: 1468, 8: 1644, 16: 1836}
     T = N // 16
     lane_instr = L * (2 * N) ** 2 * T * P3_FP64_PER_THREAD_TILE[T]
     roofline["p3_limits"] = {
         "fp64_lane_instr_per_launch": lane_instr,
         "fp64_achieved_T_per_s": lane_instr / (stage_ms["P3_z_conv"] * 1e-3) / 1e12,
         "fp64_peak_T_per_s": 18.4, "fp64_frac": lane_instr / (stage_ms["P3_z_conv"] * 1e-3) / 18.4e12,
-        "note": "P3 is co-limited by the fp64 pipe and the shared-memory data pipe (ncu: 61 % and ~65-70 % busy at "
-                "config 5, profiles/r01c), both above its HBM time; frac above is against HBM as north_star asks"}
+        "note": "P3 is co-limited by the fp64 pipe and the shared-memory data pipe (ncu: 66 % and ~60-65 % busy at "
+                "config 5, profiles/r01d), both above its HBM time; frac above is against HBM as north_star asks"}
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")   # written by hand from an ncu --set full capture
     if os.path.exists(traffic_file):
         try:
