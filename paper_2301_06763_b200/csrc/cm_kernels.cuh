@@ -648,6 +648,9 @@ struct AccelField {
 
 // the general (face / cavity) case of one pair of cells, kept out of line so that the streaming
 // loop of k_accel stays small in registers
+// the one ghost value beyond an x face, out of line as well
+__device__ __noinline__ double accel_ghost_x(const AccelField F, int k, int j, int i) { return F.ghost(k, j, i, 0); }
+
 __device__ __noinline__ void accel_pair_general(const AccelField F, int k, int j, int i, double inv, double2 &gx,
                                                 double2 &gy, double2 &gz)
 {
@@ -676,7 +679,10 @@ __global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, 
     const double *pl = phi + (size_t)l * n3;
     const bool has_cav = l < L - 1;
     const AccelField F{pl, l > 0 ? phi + (size_t)(l - 1) * n3 : nullptr, has_cav ? pbar + (size_t)l * h3 : nullptr, N};
-    const bool inner_ji = j >= 1 && j <= N - 2 && i >= 2 && i <= N - 4;
+    // fast path: every y/z neighbour inside the grid and nothing under the finer grid; at the two x ends of a row only
+    // the one missing x neighbour is a ghost (a row is 1-4 warps: sending those warps down the general path for one
+    // lane each cost half of the kernel's time)
+    const bool inner_ji = j >= 1 && j <= N - 2;
     const bool cav_ji = has_cav && j >= Q - 1 && j <= 3 * Q && i >= Q - 2 && i <= 3 * Q;
     const size_t rji = (size_t)j * N + i;
     double2 zm = make_double2(0.0, 0.0), c = *reinterpret_cast<const double2 *>(pl + (size_t)k0 * nn + rji);
@@ -689,7 +695,7 @@ __global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, 
         if (k + 1 < N) zp = *reinterpret_cast<const double2 *>(pl + r + nn);
         double2 gx, gy, gz;
         if (inner_ji && k >= 1 && k <= N - 2 && !(cav_ji && k >= Q - 1 && k <= 3 * Q)) {
-            const double xm = pl[r - 1], xp = pl[r + 2];
+            const double xm = i > 0 ? pl[r - 1] : accel_ghost_x(F, k, j, -1), xp = i + 2 < N ? pl[r + 2] : accel_ghost_x(F, k, j, N);
             const double2 ym = *reinterpret_cast<const double2 *>(pl + r - N), yp = *reinterpret_cast<const double2 *>(pl + r + N);
             gx = make_double2(-(c.y - xm) * inv, -(xp - c.x) * inv);
             gy = make_double2(-(yp.x - ym.x) * inv, -(yp.y - ym.y) * inv);
