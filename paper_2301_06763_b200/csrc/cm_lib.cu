@@ -46,7 +46,8 @@ struct cm_plan {
     int launches = 0;
     int num_sms = 148;
     int zconv_grid = 0;
-    CUtensorMap mapW;
+    CUtensorMap mapW, mapWw;        // W2 as CTA-wide 128-byte boxes / as per-warp 32- or 64-byte boxes (k_z_conv_warp)
+    bool zconv_warp = false;
     int kernels_per_solve = 0;
     bool fused_fwd = false;         // P1+P2 as one persistent kernel (cm_fused.cuh), N >= 128, CM_FUSE=1
     int fuse_R = 0, fuse_LAG = 0, fuse_grid = 0;
@@ -86,6 +87,8 @@ template <int T> int set_attrs(cm_plan *p)
         CM_CUDA(p, cudaFuncSetAttribute(k_xy_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                     (int)(smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>())));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
+    if constexpr (T >= 8)
+        CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_warp<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZWarpCfg<T>::SMEM));
     return CM_OK;
 }
 
@@ -98,6 +101,12 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
     const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
     int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
     if (p->zconv_grid > 0 && p->zconv_grid < grid) grid = p->zconv_grid;
+    if constexpr (T >= 8) {
+        if (p->zconv_warp) {
+            k_z_conv_warp<T><<<grid, kThreads, ZWarpCfg<T>::SMEM, s>>>(p->mapWw, p->Khat, p->tw, L, ngroups, b0);
+            return;
+        }
+    }
     k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0);
 }
 
@@ -258,6 +267,19 @@ int make_tensor_maps(cm_plan *p)
             return CM_ECUDA;
         }
     }
+    if (p->N >= 128) {   // per-warp boxes: PPW pencils (32 B at N = 256, 64 B at N = 128) x N rows, swizzle = the row width
+        const int ppw = 32 / (p->N / 16);
+        const cuuint64_t dims[2] = {2 * NN * NN, L * N};
+        const cuuint64_t strides[1] = {NN * NN * 16};
+        const cuuint32_t box[2] = {(cuuint32_t)(2 * ppw), (cuuint32_t)N};
+        CUresult r = enc(&p->mapWw, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, p->W2, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         ppw == 2 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) {
+            std::snprintf(p->err, sizeof(p->err), "cuTensorMapEncodeTiled(W2, per-warp boxes) failed: %d", (int)r);
+            return CM_ECUDA;
+        }
+    }
     return CM_OK;
 }
 
@@ -338,6 +360,9 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         p->split_y = sy ? sy[0] == '1' : (N == 256);   // measured: -5 % at N = 256, neutral or worse below
         const char *sxe = std::getenv("CM_SPLIT_X");
         p->split_x = sxe ? sxe[0] == '1' : (N == 256);   // measured: -14 % at N = 256, +6 % at N = 128
+        const char *zw = std::getenv("CM_ZCONV");
+        // warp-autonomous P3: -6 % at N = 128 (64-byte boxes); at N = 256 its 32-byte boxes make TMA crawl (18 ms)
+        p->zconv_warp = zw ? std::strcmp(zw, "warp") == 0 : (N == 128);
         const char *zg = std::getenv("CM_ZCONV_GRID");
         p->zconv_grid = zg ? std::atoi(zg) : 0;
         int dev = 0;

@@ -257,4 +257,157 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
 }
 
 
+template <int T> struct ZWarpCfg {
+    using C = ZConvCfg<T>;
+    static constexpr int PPW = C::PPW;
+    static constexpr uint32_t WIN = C::N * PPW * 16;                                   // a warp's input box
+    static constexpr uint32_t EXW = ((PPW * LayRow<T>::PS * 16 + 1023) / 1024) * 1024;   // a warp's exchange region / output box
+    static constexpr uint32_t OFF_IN = 0, OFF_KH = 4 * WIN, OFF_EX = ((OFF_KH + C::KH_BYTES + 1023) / 1024) * 1024,
+                              OFF_TW = OFF_EX + 4 * EXW, OFF_BAR = OFF_TW + C::TW_BYTES;
+    static constexpr uint32_t SMEM = OFF_BAR + 64 + 1024;
+};
+
+// ====================== P3, warp-autonomous variant (T = 8, 16) ==========================
+// The same tile, but every warp owns its PPW pencils end to end: its own TMA box ([N rows][PPW*16 B], 32B/64B
+// swizzle: conflict-free for the j-fastest reads), its own full/empty handshakes, its own output box staged in its
+// own exchange region.  No CTA-wide barrier is left in the tile loop (r01d: 9 % of the stall samples sat at the
+// three __syncthreads of a tile, 5 % at the TMA waits behind them), and the four warps drift apart, so that one
+// warp's exchanges fall under another warp's butterflies.  Only the K-hat tile is shared: a warp reports when it
+// is through with a group's tile (bar_kfree, 4 arrivals), warp 0 then fetches the next one.
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+template <int T>
+__global__ void __launch_bounds__(kThreads, 2)
+k_z_conv_warp(const __grid_constant__ CUtensorMap mapWw, const double *__restrict__ Kt, const double2 *__restrict__ tw, int L,
+              int ngroups, int b0)
+{
+    using C = ZConvCfg<T>;
+    using W = ZWarpCfg<T>;
+    constexpr int N = C::N, PEN = C::PEN, PPW = C::PPW, ROWB = PPW * 16;     // bytes of one z row of a warp's box
+    constexpr uint32_t WIN = W::WIN, EXW = W::EXW;
+    using Lay = LayRow<T>;
+    static_assert(T == 8 || T == 16, "one 32- or 64-byte box per warp");
+    static_assert(PPW * Lay::PS * 16 >= (int)WIN, "a warp's exchange region doubles as its output stage");
+    extern __shared__ unsigned char smem_raw[];
+    const uint32_t s0 = (smem_u32(smem_raw) + 1023u) & ~1023u;
+    unsigned char *sbase = smem_raw + (s0 - smem_u32(smem_raw));
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31, j = lane % T, pxl = lane / T;
+    const uint32_t bar_in = s0 + W::OFF_BAR + 8 * w, bar_k = s0 + W::OFF_BAR + 32, bar_kfree = bar_k + 8;
+    double2 *tw_s = reinterpret_cast<double2 *>(sbase + W::OFF_TW);
+    const int pen = w * PPW + pxl;
+
+    if ((int)blockIdx.x >= ngroups) return;
+    const int my_groups = (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int ntiles = my_groups * L;
+    auto tile_of = [&](int t, int &g, int &b) {
+        const int gi = t / L;
+        b = t - gi * L;
+        g = (int)blockIdx.x + gi * (int)gridDim.x;
+    };
+    const uint32_t in_u = s0 + W::OFF_IN + w * WIN, ex_u = s0 + W::OFF_EX + w * EXW;
+    unsigned char *in_p = sbase + W::OFF_IN + w * WIN, *out_p = sbase + W::OFF_EX + w * EXW;
+    double2 *ex_p = reinterpret_cast<double2 *>(out_p) + pxl * Lay::PS;
+    auto issue_in = [&](int g, int b) {       // lane 0 of the warp
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(bar_in, WIN);
+        tma_load_2d(in_u, &mapWw, 2 * (g * PEN + w * PPW), (b0 + b) * N, bar_in);
+    };
+    auto issue_k = [&](int g) {               // thread 0
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(bar_k, C::KH_BYTES);
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(s0 + W::OFF_KH),
+                     "l"(Kt + (size_t)g * PEN * C::RSK), "r"(C::KH_BYTES), "r"(bar_k)
+                     : "memory");
+    };
+    if (tid == 0) {
+        for (int q = 0; q < 4; ++q) mbar_init(s0 + W::OFF_BAR + 8 * q, 1);
+        mbar_init(bar_k, 1);
+        mbar_init(bar_kfree, 4);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = tid; i < 32 * T; i += kThreads) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
+    __syncthreads();
+    {
+        int g0, bb0;
+        tile_of(0, g0, bb0);
+        if (tid == 0) issue_k(g0);
+        if (lane == 0) issue_in(g0, bb0);
+    }
+    const double *kh_p = reinterpret_cast<const double *>(sbase + W::OFF_KH) + pen * C::RSK;
+    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j], tw_s[4 * T + j], tw_s[6 * T + j]};
+    // swizzled position of (row z, pencil pxl) in a warp's box: 32B rows: chunk bit0 ^= bit 7 of the offset;
+    // 64B rows: chunk bits [1:0] ^= bits [8:7]
+    auto box_off = [&](int z) -> uint32_t {
+        const uint32_t off = (uint32_t)z * ROWB + (uint32_t)pxl * 16;
+        return ROWB == 32 ? (off ^ (((off >> 7) & 1u) << 4)) : (off ^ (((off >> 7) & 3u) << 4));
+    };
+    uint32_t ph_in = 0, ph_k = 0, ph_kfree = 0;
+
+    for (int t = 0; t < ntiles; ++t) {
+        int g, b, gn = 0, bn = 0;
+        tile_of(t, g, b);
+        if (t + 1 < ntiles) tile_of(t + 1, gn, bn);
+
+        mbar_wait(bar_in, ph_in);
+        ph_in ^= 1;
+        double2 a[16];
+#pragma unroll
+        for (int r = 0; r < 16; ++r) a[r] = *reinterpret_cast<const double2 *>(in_p + box_off(j + T * r));
+        if (lane == 0) tma_store_wait_read();     // this warp's previous output has left its exchange region
+        __syncwarp();
+        if (lane == 0 && t + 1 < ntiles) issue_in(gn, bn);
+        if (t == 0 || b == 0) {
+            mbar_wait(bar_k, ph_k);
+            ph_k ^= 1;
+        }
+        auto kmul = [&](double2(&v)[16], int P) {
+#pragma unroll
+            for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+                for (int k2 = 0; k2 < T; ++k2) {
+                    const double k = kh_p[P * N + 16 * k2 + cc * T + j];
+                    v[cc * T + k2].x *= k;
+                    v[cc * T + k2].y *= k;
+                }
+        };
+        double2 e[16];
+        {
+            {
+                double2 v[16];
+                fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncWarp());
+                kmul(v, 0);
+                inv_half<T, 0, Lay, true>(v, e, j, ex_p, tws, SyncWarp());
+            }
+            double2 v[16], o[16];
+            fwd_half<T, 1, Lay, true>(a, v, j, ex_p, tws, SyncWarp());
+            kmul(v, 1);
+            if (t + 1 < ntiles && gn != g) {      // this warp is through with the group's K-hat tile
+                __syncwarp();
+                if (lane == 0) mbar_arrive(bar_kfree);
+                if (tid == 0) {                   // warp 0 fetches the next tile once all four warps are through
+                    mbar_wait(bar_kfree, ph_kfree);
+                    ph_kfree ^= 1;
+                    issue_k(gn);
+                }
+            }
+            inv_half<T, 1, Lay, true>(v, o, j, ex_p, tws, SyncWarp());
+#pragma unroll
+            for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
+        }
+        __syncwarp();                             // the warp's exchanges are over: its region becomes the output box
+#pragma unroll
+        for (int r = 0; r < 16; ++r) *reinterpret_cast<double2 *>(out_p + box_off(j + T * r)) = e[r];
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) {
+            tma_store_2d(&mapWw, 2 * (g * PEN + w * PPW), (b0 + b) * N, ex_u);
+            tma_store_commit();
+        }
+    }
+    if (lane == 0) tma_store_wait_all();
+}
+
 }  // namespace cmk
