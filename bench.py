@@ -367,6 +367,23 @@ def run_ours(args) -> None:
             ms_mod = m0.elapsed_time(m1) / e2e_steps
             modified = {"ms": ms_mod, "ratio_to_original": ms_mod / ms_step, "pairs": L - 1,
                         "note": "cm_potential_modified: one (2N)^3 single-level convolution per pair, two pairs per complex solve"}
+
+            def _time(fn, reps):
+                fn()
+                t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                t0.record(stream)
+                for _ in range(reps):
+                    fn()
+                t1.record(stream)
+                torch.cuda.synchronize()
+                return t0.elapsed_time(t1) / reps
+
+            if N <= 64 and L > 2:       # Eq. B.3-B.6: the quadrupled grid needs 4N <= 256
+                modified["triplets_ms"] = _time(lambda: plan.potential_modified_triplets(rho, pm), e2e_steps)
+            if N <= 32 and L > 2:       # Eq. B.7 in place of the quadrupled grid, and on its own (finest -> coarsest)
+                modified["triplets_direct_ms"] = _time(lambda: plan.potential_modified_triplets(rho, pm, qdp_direct=True), 3)
+                modified["direct_sum_ms"] = _time(lambda: plan.direct_sum(rho, L - 1, 0), 3)
             del pm
         except Exception as e:
             modified = {"error": str(e)}
