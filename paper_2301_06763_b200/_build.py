@@ -8,7 +8,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libcm.so")
 SOURCES = ["cm_lib.cu"]
-DEPS = ["cm_lib.cu", "cm_kernels.cuh", "cm_zconv.cuh", "cm_fused.cuh", "cm_fft.cuh", os.path.join("..", "..", "include", "cm.h")]
+DEPS = ["cm_lib.cu", "cm_kernels.cuh", "cm_zconv.cuh", "cm_fft.cuh", os.path.join("..", "..", "include", "cm.h")]
 
 # no --use_fast_math: fp64 parity needs IEEE division and sqrt
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -60,8 +60,6 @@ template <int T> struct LayRow {
 
 struct SyncBlock { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
 struct SyncWarp  { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
-// the kThreads compute threads of a CTA that also carries a scheduler warp (cm_fused.cuh)
-struct SyncCompute { __device__ __forceinline__ void operator()() const { asm volatile("bar.sync 1, 128;" ::: "memory"); } };
 
 // ---- twiddle sources ------------------------------------------------------------------
 // w_2N^{j (2 k1 + P)}: from the global table (read-only path) or from a per-CTA shared copy
@@ -83,11 +81,7 @@ template <int T> struct TwShared {
     double2 rho;           // w_2N^{2 j}
     double2 rho2, rho3;    // w_2N^{4 j}, w_2N^{6 j}
     static constexpr bool RECUR = true;
-#ifndef ABL_NOTW
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return base[(2 * k1 + P) * T]; }
-#else
-    template <int P> __device__ __forceinline__ double2 get(int k1) const { return make_double2(0.6 + k1, 0.8 - P); }
-#endif
     __device__ __forceinline__ double2 step() const { return rho; }
     __device__ __forceinline__ double2 step2() const { return rho2; }
     __device__ __forceinline__ double2 step3() const { return rho3; }
@@ -123,22 +117,13 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
             if (k1 > 0 || P) b[k1] = cmul(b[k1], tw_next<P>(tw, k1, twp));
-#ifndef ABL_NOEX
             sm[k1 * Lay::RS + j] = b[k1];
-#endif
         }
-#ifndef ABL_NOEX
         sync();
-#endif
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc) {
-#ifndef ABL_NOEX
 #pragma unroll
             for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = sm[(cc * T + j) * Lay::RS + jj];
-#else
-#pragma unroll
-            for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = b[cc * T + jj];
-#endif
             Dft<T, -1>::run(&v[cc * T]);
         }
     } else {
@@ -158,22 +143,14 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc) {
             Dft<T, +1>::run(&v[cc * T]);
-#ifndef ABL_NOEX
 #pragma unroll
             for (int jj = 0; jj < T; ++jj) sm[(cc * T + j) * Lay::RS + jj] = v[cc * T + jj];
-#endif
         }
-#ifndef ABL_NOEX
         sync();
-#endif
         double2 twp = make_double2(1.0, 0.0);
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
-#ifndef ABL_NOEX
             o[k1] = sm[k1 * Lay::RS + j];
-#else
-            o[k1] = v[k1];
-#endif
             if (k1 > 0 || P) o[k1] = cmulc(o[k1], tw_next<P>(tw, k1, twp));
         }
     } else {
@@ -290,8 +267,17 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_x_fwd_split(const double *_
 //     Phi(Omega_b) = Phi^b + ext_b               (Eq. 14)
 // and hole_b = Phi_hole^b + ext_b is kept where the next level will read it (on every cell if hole_all:
 // the modified method, Eq. B.1, builds Phi(Omega_b) from it).
+//
+// The L launches are chained by programmatic dependent launch: a level's CTAs let the next level start as soon as
+// they are all resident (griddepcontrol.launch_dependents at the top), and only the fetch of Hc — the one thing that
+// needs the level before — sits behind griddepcontrol.wait.  So level b+1 loads its spectrum and runs its inverse
+// transforms under the tail of level b instead of after it (at N <= 128 a level is a wave or less: without this
+// the levels ran one after the other on a partly empty GPU).  W1 is complete before level 0 starts (a normal launch).
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 template <int T>
-__global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
+__global__ void __launch_bounds__(kThreads, T >= 8 ? 3 : 2) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
                                                     double *__restrict__ hole, const double *__restrict__ hole_c,
                                                     const double2 *__restrict__ tw, int L, double scale0 /* -G dx0^2 */,
                                                     size_t row0, int hole_all, double *__restrict__ phi_im)
@@ -299,25 +285,34 @@ __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ 
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, Q = N / 4;
     using Lay = LayRow<T>;
     extern __shared__ double2 smem[];
+    pdl_launch_dependents();
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
     const size_t rowc = (size_t)blockIdx.x * ROWS + rowl, row = row0 + rowc;
     const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
     const double2 *src = W1 + row * NN;
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
 
-    double2 v0[16], v1[16];
+    double2 e[16];
+    {
+        double2 v0[16], v1[16], o[16];
 #pragma unroll
-    for (int cc = 0; cc < 16 / T; ++cc)
+        for (int cc = 0; cc < 16 / T; ++cc)
 #pragma unroll
-        for (int k2 = 0; k2 < T; ++k2) {
-            v0[cc * T + k2] = src[16 * k2 + cc * T + j];
-            v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
-        }
-    // a8: the prolonged contribution of the coarser levels, fetched (from L2: the previous launch
-    // wrote it) while the row's spectrum is still on its way, so its latency hides behind the transform
+            for (int k2 = 0; k2 < T; ++k2) {
+                v0[cc * T + k2] = src[16 * k2 + cc * T + j];
+                v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
+            }
+        inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
+        inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncWarp());
+#pragma unroll
+        for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
+    }
+
+    // a8: the prolonged contribution of the coarser levels (L2 hits: the launch before this one wrote it)
     const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
     double ext[16];
     if (b > 0) {
+        pdl_wait();
         const double *Hc = hole_c + (size_t)(b - 1) * N * N * N;
         const int pk = Q + z / 2, pj = Q + y / 2, sk = (z & 1) ? 1 : -1, sj = (y & 1) ? 1 : -1;
         const double *h0 = Hc + ((size_t)pk * N + pj) * N, *h1 = Hc + ((size_t)(pk + sk) * N + (pj + sj)) * N;
@@ -331,16 +326,12 @@ __global__ void __launch_bounds__(kThreads) k_x_inv(const double2 *__restrict__ 
         for (int r = 0; r < 16; ++r) ext[r] = 0.0;
     }
 
-    double2 e[16], o[16];
-    inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
-    inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncWarp());
-
     const double scale = scale0 * exp2(-2.0 * b);   // dx_b^2 = dx0^2 / 4^b, exact
     double *dphi = phi + row * N, *dh = hole + row * N;
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
         const int x = j + T * r;
-        const double re = scale * (e[r].x + o[r].x), im = scale * (e[r].y + o[r].y);
+        const double re = scale * e[r].x, im = scale * e[r].y;
         dphi[x] = b > 0 ? re + ext[r] : re;
         if (hole_all ? (b < L - 1) : (rowring && in_ring1(x, N))) dh[x] = b > 0 ? im + ext[r] : im;
         if (phi_im) phi_im[row * N + x] = im;       // the second field of a dual single-level solve

@@ -11,16 +11,16 @@
 #include "../../include/cm.h"
 #include "cm_kernels.cuh"
 #include "cm_zconv.cuh"
-#include "cm_fused.cuh"
 
 namespace {
 
 struct GraphEntry {
     const double *rho;
     double *phi;
-    cudaGraph_t graph;
     cudaGraphExec_t exec;
+    unsigned long long last_use;   // for least-recently-used eviction
 };
+constexpr size_t kGraphCacheSize = 8;
 
 }  // namespace
 
@@ -32,7 +32,7 @@ struct cm_plan {
     double *stage_rho = nullptr, *stage_phi = nullptr;
     size_t bytes = 0;
     bool green_ready = false;
-    bool split_x = false, split_y = false;   // P1 / P2 split by output parity (256-thread CTAs): default at N = 256
+    bool split_x = false, split_y = false;   // P1 / P2 split by output parity (256-thread CTAs): N = 256
     int hole_all = 0;               // P5 keeps Phi_hole + ext on every cell (cm_potential_modified)
     cm_plan *dbl = nullptr, *qdp = nullptr;   // single-level plans of the doubled (2N)^3 and quadrupled (4N)^3 fine grid
     double *rho4 = nullptr, *phi4 = nullptr, *tmp3 = nullptr;
@@ -43,16 +43,12 @@ struct cm_plan {
     cudaStream_t cap_stream = nullptr, copy_stream = nullptr;
     std::vector<cudaEvent_t> ev_level;   // cm_potential_host's pipeline: [0,32) level arrived, [32,64) level's Phi ready, [64] start
     std::vector<GraphEntry> graphs;
+    unsigned long long use_counter = 0;
     int launches = 0;
     int num_sms = 148;
-    int zconv_grid = 0;
     CUtensorMap mapW, mapWw;        // W2 as CTA-wide 128-byte boxes / as per-warp 32- or 64-byte boxes (k_z_conv_warp)
     bool zconv_warp = false;
     int kernels_per_solve = 0;
-    bool fused_fwd = false;         // P1+P2 as one persistent kernel (cm_fused.cuh), N >= 128, CM_FUSE=1
-    int fuse_R = 0, fuse_LAG = 0, fuse_grid = 0;
-    cmk::FusedCtl *ctl = nullptr;
-    size_t ctl_bytes = 0;
     char err[512] = {0};
 };
 
@@ -83,9 +79,6 @@ template <int T> int set_attrs(cm_plan *p)
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_occ3<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-    if constexpr (T >= 8)
-        CM_CUDA(p, cudaFuncSetAttribute(k_xy_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    (int)(smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>())));
     CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
     if constexpr (T >= 8)
         CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_warp<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZWarpCfg<T>::SMEM));
@@ -99,8 +92,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
     const int ngroups = NN * NN / ZConvCfg<T>::PEN;
     // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
     const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
-    int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
-    if (p->zconv_grid > 0 && p->zconv_grid < grid) grid = p->zconv_grid;
+    const int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
     if constexpr (T >= 8) {
         if (p->zconv_warp) {
             k_z_conv_warp<T><<<grid, kThreads, ZWarpCfg<T>::SMEM, s>>>(p->mapWw, p->Khat, p->tw, L, ngroups, b0);
@@ -108,6 +100,27 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
         }
     }
     k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0);
+}
+
+// P5 of level b.  chained: programmatic dependent launch on the launch before it in the stream (level b-1's P5), so
+// that this level's loads and transforms overlap that level's tail; the kernel waits (griddepcontrol.wait) only
+// before it reads what level b-1 wrote.
+template <int T>
+void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid, double scale0, double *phi_im, bool chained)
+{
+    constexpr int N = 16 * T;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = smem_row<T>();
+    cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = chained ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, k_x_inv<T>, (const double2 *)p->W1, phi, p->hole, (const double *)p->hole, (const double2 *)p->tw, p->L,
+                       scale0, (size_t)b * N * N, p->hole_all, phi_im);
 }
 
 // The five FFT passes (steps a3-a7) with the prolongation + Eq. 14 sum (a8) folded into P5:
@@ -119,25 +132,12 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     const int L = p->L;
     const size_t planes = (size_t)L * N;
     const double scale0 = -p->G * p->dx0 * p->dx0;
-    bool fused_done = false;
-    if constexpr (T >= 8) {
-    if (p->fused_fwd) {
-        fused_done = true;
-        // P1 and P2 interleave inside one persistent kernel: reported together under P2
-        if (ev) cudaEventRecord(ev[2], s);
-        cudaMemsetAsync(p->ctl, 0, p->ctl_bytes, s);
-        const size_t sm = smem_row<T>() > smem_batch<T>() ? smem_row<T>() : smem_batch<T>();
-        k_xy_fwd<T><<<p->fuse_grid, kThreads + 32, sm, s>>>(rho, p->rc, p->W1, p->W2, p->tw, L, p->ctl, p->fuse_R, p->fuse_LAG);
-    }
-    }
-    if (!fused_done) {
-        if (p->split_x && !p->dual_in) k_x_fwd_split<T><<<(unsigned)(planes * N / ROWS), 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
-        else k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
-        if (ev) cudaEventRecord(ev[2], s);
-        if (p->split_y) k_y_fwd_split<T><<<(unsigned)(planes * NN / PEN), 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
-        else if (T == 16) k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
-        else k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
-    }
+    if (p->split_x && !p->dual_in) k_x_fwd_split<T><<<(unsigned)(planes * N / ROWS), 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
+    else k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
+    if (ev) cudaEventRecord(ev[2], s);
+    if (p->split_y) k_y_fwd_split<T><<<(unsigned)(planes * NN / PEN), 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    else if (T == 16) k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    else k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     if (ev) cudaEventRecord(ev[3], s);
     launch_zconv<T>(p, s, 0, L);
     if (ev) cudaEventRecord(ev[4], s);
@@ -145,10 +145,9 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     if (ev) cudaEventRecord(ev[5], s);
     const size_t lrows = (size_t)N * N;
     const unsigned gl = (unsigned)((lrows + ROWS - 1) / ROWS);
-    for (int b = 0; b < L; ++b)
-        k_x_inv<T><<<gl, kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, L, scale0, (size_t)b * lrows, p->hole_all, p->dual_out);
+    for (int b = 0; b < L; ++b) launch_x_inv<T>(p, phi, s, b, gl, scale0, p->dual_out, /*chained=*/b > 0);
     if (ev) cudaEventRecord(ev[6], s);
-    p->launches += (p->fused_fwd ? 3 : 4) + L;
+    p->launches += 4 + L;
     CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
@@ -170,8 +169,7 @@ template <int T> void level_p5(cm_plan *p, double *phi, cudaStream_t s, int l)
 {
     constexpr int N = 16 * T, ROWS = kThreads / T;
     const size_t lrows = (size_t)N * N;
-    k_x_inv<T><<<(unsigned)((lrows + ROWS - 1) / ROWS), kThreads, smem_row<T>(), s>>>(p->W1, phi, p->hole, p->hole, p->tw, p->L,
-                                                                                   -p->G * p->dx0 * p->dx0, (size_t)l * lrows, p->hole_all, nullptr);
+    launch_x_inv<T>(p, phi, s, l, (unsigned)((lrows + ROWS - 1) / ROWS), -p->G * p->dx0 * p->dx0, nullptr, /*chained=*/false);
 }
 void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int l, bool p5)
 {
@@ -215,10 +213,8 @@ int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cu
 
 void destroy_graphs(cm_plan *p)
 {
-    for (auto &g : p->graphs) {
+    for (auto &g : p->graphs)
         if (g.exec) cudaGraphExecDestroy(g.exec);
-        if (g.graph) cudaGraphDestroy(g.graph);
-    }
     p->graphs.clear();
 }
 
@@ -302,9 +298,14 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
     p->L = levels;
     p->T = N / 16;
     p->dx0 = dx0;
-    const char *ng = std::getenv("CM_NO_GRAPH");
-    p->use_graph = !(ng && ng[0] == '1');
-
+    // the one environment switch (cm.h): CM_DEBUG=nograph launches kernel by kernel instead of through a CUDA graph
+    if (const char *dbg = std::getenv("CM_DEBUG")) {
+        if (std::strcmp(dbg, "nograph") == 0) p->use_graph = false;
+        else if (dbg[0] != '\0') {
+            delete p;
+            return CM_EINVAL;
+        }
+    }
     const size_t n = 2 * (size_t)N, n3 = (size_t)N * N * N, h3 = n3 / 8, L = (size_t)levels;
     int rc = CM_OK;
     if ((rc = dev_alloc(p, &p->W1, L * N * N * n)) == CM_OK &&
@@ -333,38 +334,10 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
             rc = CM_ECUDA;
     }
     if (rc == CM_OK) {
-        // fused P1+P2: ring and lag in planes from the number of tickets in flight (cm_fused.cuh)
-        const char *ef = std::getenv("CM_FUSE");
-        p->fused_fwd = (N >= 128) && (ef && ef[0] == '1');   // off by default: correct, 40 % fewer DRAM bytes, but latency-bound
-        int dev = 0, sms = 148;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        const int T = N / 16, per = N >= 128 ? N / (kThreads / T) + 2 * N / (8 * (16 / T)) : 1;
-        p->fuse_grid = 2 * sms;
-        const int span = (p->fuse_grid + per - 1) / per;
-        p->fuse_LAG = span + 1;
-        p->fuse_R = p->fuse_LAG + span + 2;
-        const char *el = std::getenv("CM_FUSE_LAG"), *er = std::getenv("CM_FUSE_R"), *eg = std::getenv("CM_FUSE_GRID");
-        if (el) p->fuse_LAG = std::atoi(el);
-        if (er) p->fuse_R = std::atoi(er);
-        if (eg) p->fuse_grid = std::atoi(eg);
-        if (p->fuse_R <= p->fuse_LAG) p->fuse_R = p->fuse_LAG + 1;
-        if ((size_t)p->fuse_R > L * N) p->fused_fwd = false;
-        p->ctl_bytes = sizeof(FusedCtl) + 2 * L * N * sizeof(unsigned);
-        void *q = nullptr;
-        if (cuda_fail(p, cudaMalloc(&q, p->ctl_bytes), "cudaMalloc(ctl)")) rc = CM_ECUDA;
-        p->ctl = (cmk::FusedCtl *)q;
-    }
-    if (rc == CM_OK) {
-        const char *sy = std::getenv("CM_SPLIT_Y");
-        p->split_y = sy ? sy[0] == '1' : (N == 256);   // measured: -5 % at N = 256, neutral or worse below
-        const char *sxe = std::getenv("CM_SPLIT_X");
-        p->split_x = sxe ? sxe[0] == '1' : (N == 256);   // measured: -14 % at N = 256, +6 % at N = 128
-        const char *zw = std::getenv("CM_ZCONV");
-        // warp-autonomous P3: -6 % at N = 128 (64-byte boxes); at N = 256 its 32-byte boxes make TMA crawl (18 ms)
-        p->zconv_warp = zw ? std::strcmp(zw, "warp") == 0 : (N == 128);
-        const char *zg = std::getenv("CM_ZCONV_GRID");
-        p->zconv_grid = zg ? std::atoi(zg) : 0;
+        // kernel variants by size, each chosen by measurement
+        p->split_y = (N == 256);      // P2 split by output parity: -5 % at N = 256, neutral or worse below
+        p->split_x = (N == 256);      // P1 split by output parity: -14 % at N = 256, +6 % at N = 128
+        p->zconv_warp = (N == 128);   // warp-autonomous P3: -6 % at N = 128; at N = 256 its 32-byte TMA boxes crawl
         int dev = 0;
         if (cuda_fail(p, cudaGetDevice(&dev), "cudaGetDevice") ||
             cuda_fail(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
@@ -385,7 +358,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         return rc;
     }
     // number of kernels per solve: (L-1) restrictions + P1..P4 + one P5 per level
-    p->kernels_per_solve = (levels - 1) + (p->fused_fwd ? 3 : 4) + levels;
+    p->kernels_per_solve = (levels - 1) + 4 + levels;
     p->launches = p->kernels_per_solve;
     *out = p;
     return CM_OK;
@@ -432,22 +405,34 @@ int cm_potential(cm_plan *p, const double *rho, double *phi, void *stream)
 
     for (auto &g : p->graphs)
         if (g.rho == rho && g.phi == phi) {
+            g.last_use = ++p->use_counter;
             CM_CUDA(p, cudaGraphLaunch(g.exec, s));
             return CM_OK;
         }
-    // capture once per (rho, phi) pair on the plan's own stream, launch on the caller's
-    GraphEntry ge{rho, phi, nullptr, nullptr};
+    // capture once per (rho, phi) pair on the plan's own stream, launch on the caller's; the cache keeps the
+    // kGraphCacheSize most recently used pairs (callers that rotate buffers should reuse them)
+    cudaGraph_t graph = nullptr;
     CM_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
     const int rc = enqueue_solve(p, rho, phi, p->cap_stream);
-    cudaError_t ee = cudaStreamEndCapture(p->cap_stream, &ge.graph);
-    if (rc != CM_OK) {
-        if (ge.graph) cudaGraphDestroy(ge.graph);
-        return rc;
+    cudaError_t ee = cudaStreamEndCapture(p->cap_stream, &graph);
+    if (rc != CM_OK || ee != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        if (rc != CM_OK) return rc;
+        CM_CUDA(p, ee);
     }
+    GraphEntry ge{rho, phi, nullptr, ++p->use_counter};
+    ee = cudaGraphInstantiate(&ge.exec, graph, 0);
+    cudaGraphDestroy(graph);   // the executable graph is self-contained
     CM_CUDA(p, ee);
-    CM_CUDA(p, cudaGraphInstantiate(&ge.exec, ge.graph, 0));
-    if (p->graphs.size() >= 8) destroy_graphs(p);
-    p->graphs.push_back(ge);
+    if (p->graphs.size() >= kGraphCacheSize) {
+        size_t lru = 0;
+        for (size_t i = 1; i < p->graphs.size(); ++i)
+            if (p->graphs[i].last_use < p->graphs[lru].last_use) lru = i;
+        cudaGraphExecDestroy(p->graphs[lru].exec);
+        p->graphs[lru] = ge;
+    } else {
+        p->graphs.push_back(ge);
+    }
     CM_CUDA(p, cudaGraphLaunch(ge.exec, s));
     return CM_OK;
 }
@@ -537,14 +522,23 @@ namespace {
 // one expanded-grid plan (N' = F N, one level, unit G and dx) with room for two fields (dual solve)
 int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **rho_big, double **phi_big)
 {
-    if (*plan) return CM_OK;
+    if (*plan && *rho_big && *phi_big) return CM_OK;
     const size_t n3 = (size_t)p->N * p->N * p->N, big = (size_t)F * F * F * n3;
-    int rc = cm_plan_create(plan, F * p->N, 1, 1.0, 2);
+    const size_t keep = p->bytes;
+    int rc = CM_OK;
+    if (!*plan) rc = cm_plan_create(plan, F * p->N, 1, 1.0, 2);
     if (rc == CM_OK) rc = cm_green_precompute(*plan);
-    if (rc == CM_OK) rc = dev_alloc(p, rho_big, 2 * big);
-    if (rc == CM_OK) rc = dev_alloc(p, phi_big, 2 * big);
+    if (rc == CM_OK && !*rho_big) rc = dev_alloc(p, rho_big, 2 * big);
+    if (rc == CM_OK && !*phi_big) rc = dev_alloc(p, phi_big, 2 * big);
     if (rc != CM_OK) {
+        // all or nothing: a later call must not find a half-built expanded plan
         if (*plan) std::snprintf(p->err, sizeof(p->err), "expanded-grid plan (x%d): %.400s", F, (*plan)->err);
+        cm_plan_destroy(*plan);
+        *plan = nullptr;
+        cudaFree(*rho_big);
+        cudaFree(*phi_big);
+        *rho_big = *phi_big = nullptr;
+        p->bytes = keep;
         return rc;
     }
     p->bytes += (*plan)->bytes;
@@ -725,7 +719,6 @@ int cm_plan_destroy(cm_plan *p)
     cudaFree(p->rho4);
     cudaFree(p->phi4);
     cudaFree(p->tmp3);
-    cudaFree(p->ctl);
     cudaFree(p->tw);
     cudaFree(p->stage_rho);
     cudaFree(p->stage_phi);

@@ -167,16 +167,8 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
     const unsigned char *in_p = sbase + C::OFF_IN + bx * (N * 128);
     const double *kh_p = reinterpret_cast<const double *>(sbase + C::OFF_KH) + pen * C::RSK;
     double2 *ex_p = ex_s + pen * Lay::PS;
-#ifdef ZC_TWGLOBAL
-    const TwGlobal tws{tw, j};
-#else
     const TwShared<T> tws{tw_s + j, tw_s[2 * T + j], tw_s[4 * T + j], tw_s[6 * T + j]};
-#endif
-#ifdef ZC_SYNCBLOCK
-    using SyncX = SyncBlock;
-#else
     using SyncX = SyncWarp;
-#endif
     uint32_t ph_in = 0, ph_k = 0;
 
     for (int t = 0; t < ntiles; ++t) {
@@ -236,25 +228,21 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
                 const int z = j + T * r;
-#ifdef ZC_NOSTORE
-                if (e[r].x == 1.2345e-300)
-#endif
                 *reinterpret_cast<double2 *>(out_p + z * 128 + ((px ^ (z & 7)) << 4)) = e[r];
             }
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
         if (tid == 0) {
-#ifndef ZC_NOSTORE
 #pragma unroll
             for (int q = 0; q < NBOX; ++q)
                 tma_store_2d(&mapW, 2 * (g * PEN + 8 * q), (b0 + b) * N, s0 + C::OFF_EX + q * (N * 128));
             tma_store_commit();
-#endif
         }
     }
     if (tid == 0) tma_store_wait_all();
 }
+
 
 
 template <int T> struct ZWarpCfg {

@@ -123,6 +123,20 @@ def test_config5_full_size_sampled_and_invariants():
         assert np.abs(gm[l, 1][:, :, ::-1] - g[l, 1]).max() <= TOL * s
 
 
+def test_config5_size_every_cell_against_the_oracle():
+    """10 x 256^3, every cell of every level and component (ZCH/TX/TY of k_accel differ from the N <= 64 cases):
+    the numpy oracle is cheap enough for the whole grid."""
+    N, L = 256, 10
+    rng = np.random.default_rng(256)
+    phi = rng.standard_normal((L, N, N, N))
+    dx0 = 0.37 / N
+    g = _gpu_accel(phi, dx0)
+    ref = oracle.acceleration(phi, dx0)
+    _assert_parity(g, ref)
+    errs = [float(np.abs(g[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(L)]
+    print("PARITY cm_acceleration 10 x 256^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))
+
+
 def test_error_codes():
     import paper_2301_06763_b200 as pkg
     plan = pkg.Plan(16, 2, 0.125)

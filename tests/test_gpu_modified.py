@@ -83,6 +83,21 @@ def test_largest_supported_grid_sampled_against_the_oracle_parts():
         assert abs(got[0][k, j, i] - ref) <= TOL * np.abs(got[0]).max(), (k, j, i)
 
 
+@pytest.mark.parametrize("L", [2, 3])
+def test_n128_every_cell_against_the_oracle(L):
+    """N = 128 (doubled grid 256^3 -> the N' = 256 kernels; L = 3: two doubled grids share one complex solve, the
+    dual path on the 256^3 plan): every cell of every level against oracle.solve_modified (its naive FFT on the
+    512^3 padded mesh, about 1.5 s per doubled field on 16 host threads)."""
+    N, dx0 = 128, 2.0 / 128
+    rng = np.random.default_rng(1280 + L)
+    rho = rng.random((L, N, N, N)) * (8.0 ** np.arange(L))[:, None, None, None]
+    got, orig = _gpu(rho, dx0, G=1.3)
+    ref = oracle.solve_modified(rho, dx0, G=1.3)
+    _assert_parity(got, ref)
+    errs = [float(np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(L)]
+    print(f"PARITY cm_potential_modified {L} x 128^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))
+
+
 def test_error_codes():
     import paper_2301_06763_b200 as pkg
     plan = pkg.Plan(256, 1, 0.1)

@@ -186,6 +186,45 @@ def test_config5_full_size_sampled_outputs_and_invariants():
     plan.close()
 
 
+def _per_level_report(tag, got, ref):
+    errs = [float(np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(ref.shape[0])]
+    print(f"PARITY {tag}: per-level max|dPhi|/max|Phi| = " + " ".join(f"{e:.2e}" for e in errs))
+    return errs
+
+
+def test_config5_whole_grid_against_the_fft_oracle():
+    """10 x 256^3, EVERY cell of every level (north_star: "all five configs"): the configuration and the launch
+    (cm_potential -> CUDA graph) bench.py times, against oracle.solve(method="fft") — 19 naive 512^3 FFT
+    convolutions on the host cores (about a minute, ~14 GB of host memory).  This is the only element-wise check of
+    the kernels that run at N = 256 only (P1/P2 split by parity, the CTA-wide TMA P3, T = 16 P4/P5)."""
+    N, L = 256, 10
+    rho = workloads.make_rho(5)
+    got, plan = _solve_gpu(rho, 2.0 / N)
+    plan.close()
+    ref = oracle.solve(rho, 2.0 / N, method="fft")
+    errs = _per_level_report("config 5 (10 x 256^3), whole grid", got, ref)
+    assert max(errs) <= TOL
+    assert np.abs(got - ref).max() / np.abs(ref).max() <= TOL
+
+
+def test_three_level_random_nest_at_256_whole_grid_and_host_entry_point():
+    """A second N = 256 case with a different structure (uniform random densities, steep level contrast), whole
+    grid; the host-buffer entry point (level pipeline: per-level launches of the N = 256 kernels, K-hat per level)
+    must give the same bits as the device entry point."""
+    pkg = _pkg()
+    N, L = 256, 3
+    rng = np.random.default_rng(2563)
+    rho = rng.random((L, N, N, N)) * (8.0 ** np.arange(L))[:, None, None, None]
+    got, plan = _solve_gpu(rho, 2.0 / N, G=0.7)
+    rho_h = torch.from_numpy(rho).pin_memory()
+    ph = plan.potential_host(rho_h)
+    assert np.array_equal(ph.numpy(), got)
+    plan.close()
+    ref = oracle.solve(rho, 2.0 / N, G=0.7, method="fft")
+    errs = _per_level_report("random 3 x 256^3, whole grid", got, ref)
+    assert max(errs) <= TOL
+
+
 # ---------------------------------------------------------------- edge cases and API behaviour
 def test_zero_density_gives_zero_potential():
     rho = np.zeros((3, 16, 16, 16))
@@ -280,26 +319,32 @@ def test_G_scales_linearly_and_error_codes():
     pkg.cm_plan_destroy(h)
 
 
-def test_fused_forward_kernel_is_bit_identical_to_the_two_pass_path(monkeypatch):
-    """CM_FUSE=1 runs P1+P2 as one persistent kernel with a W1 ring in L2 (cm_fused.cuh; not the default,
-    DESIGN.md §6).  Same arithmetic in the same order: the potentials must be bit-identical."""
+def test_graph_cache_keeps_recent_pairs_and_debug_switch(monkeypatch):
+    """More (rho, phi) pairs than the cache holds (8): least-recently-used eviction, every solve still right and
+    bit-identical; CM_DEBUG=nograph (the one environment switch, cm.h) gives the same bits kernel by kernel, an
+    unknown value is refused."""
     pkg = _pkg()
-    N, L = 128, 3
-    rho = np.random.default_rng(9).random((L, N, N, N))
-    d = torch.from_numpy(rho).cuda()
-    monkeypatch.delenv("CM_FUSE", raising=False)
-    p0 = pkg.Plan(N, L, 2.0 / N)
-    a = p0.potential(d).clone()
-    k0 = p0.kernel_launches
-    p0.close()
-    monkeypatch.setenv("CM_FUSE", "1")
-    p1 = pkg.Plan(N, L, 2.0 / N)
-    assert p1.kernel_launches == k0 - 1
-    b = p1.potential(d).clone()
-    b2 = p1.potential(d).clone()          # second solve: the control block is reset by the graph
-    p1.close()
+    N, L = 16, 2
+    rng = np.random.default_rng(12)
+    plan = pkg.Plan(N, L, 2.0 / N)
+    rhos = [torch.from_numpy(rng.random((L, N, N, N))).cuda() for _ in range(11)]
+    first = [plan.potential(r, torch.empty_like(r)).clone() for r in rhos]
+    again = [plan.potential(r, torch.empty_like(r)).clone() for r in rhos]      # new phi buffers: all re-captured
     torch.cuda.synchronize()
-    assert torch.equal(a, b) and torch.equal(a, b2)
+    for a, b in zip(first, again):
+        assert torch.equal(a, b)
+    _assert_parity(first[10].cpu().numpy(), oracle.solve(rhos[10].cpu().numpy(), 2.0 / N))
+    plan.close()
+    monkeypatch.setenv("CM_DEBUG", "nograph")
+    p2 = pkg.Plan(N, L, 2.0 / N)
+    c = p2.potential(rhos[0])
+    torch.cuda.synchronize()
+    assert torch.equal(c, first[0])
+    p2.close()
+    monkeypatch.setenv("CM_DEBUG", "bogus")
+    with pytest.raises(pkg.CMError) as ei:
+        pkg.cm_plan_create(N, L, 2.0 / N)
+    assert ei.value.code == pkg.CM_EINVAL
 
 
 def test_maximum_level_count():

@@ -98,3 +98,67 @@ def test_exchange_layouts_are_conflict_free(T):
     for cc in range(16 // T):
         for jj in range(T):
             assert _conflict_degree(row * PS + (cc * T + j) * RS + jj) == 1
+
+
+# ------------------------------------------------------------------ multi-rank host logic (replicas only), CPU, gloo
+def _rank_main(rank, world, port, out_dir):
+    import json
+    import torch
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    import bench
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+
+    def all_reduce_max(x):
+        t = torch.tensor([x], dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    ms_local = 10.0 + 5.0 * rank                       # rank 1 is the slower replica
+    agg = bench.aggregate_over_ranks(ms_local, cells_per_rank=1000, world=world, all_reduce_max=all_reduce_max)
+    assert bench.dist_env() == (rank, world, rank)
+    bench.ensure_world(world, [])                      # consistent: returns
+    with open(os.path.join(out_dir, f"rank{rank}.json"), "w") as f:
+        json.dump(agg, f)
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_replica_aggregation_over_two_gloo_ranks(tmp_path):
+    """bench.py --gpus N = N independent replicas: step time = max over ranks, value = the units all
+    ranks processed per that time.  Two CPU processes over gloo on 127.0.0.1."""
+    import json
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    mp.spawn(_rank_main, args=(2, port, str(tmp_path)), nprocs=2, join=True)
+    for r in range(2):
+        agg = json.load(open(tmp_path / f"rank{r}.json"))
+        assert agg["ms_per_step"] == 15.0                               # the slower rank decides
+        assert abs(agg["value"] - 2 * 1000 / 15e-3) < 1e-6
+        assert abs(agg["solves_per_s"] - 2 / 15e-3) < 1e-9
+
+
+def test_gpus_flag_must_match_world_size(monkeypatch):
+    sys.path.insert(0, ROOT)
+    import bench
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    with pytest.raises(SystemExit):
+        bench.ensure_world(8, [])
+    bench.ensure_world(2, [])
+    monkeypatch.delenv("WORLD_SIZE")
+    bench.ensure_world(1, [])                          # single process, nothing to do
+    assert bench.aggregate_over_ranks(4.0, 100, 1)["value"] == 100 / 4e-3
+
+
+def test_reference_arm_runs_on_rank_zero_only(monkeypatch, capsys):
+    sys.path.insert(0, ROOT)
+    import argparse
+    import bench
+    monkeypatch.setenv("RANK", "1")
+    monkeypatch.setenv("WORLD_SIZE", "2")
+    bench.run_reference(argparse.Namespace(config=1, steps=1, warmup=0, gpus=2))
+    assert capsys.readouterr().out == ""
