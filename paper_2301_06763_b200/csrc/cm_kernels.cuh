@@ -276,13 +276,17 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_x_fwd_split(const double *_
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// LATE (N <= 128): fetch Hc after the transforms, behind griddepcontrol.wait — the level overlaps the one before it.
+// N = 256 (a level is 28 waves, the overlap is worth little): wait first and fetch Hc at the top, so that its latency
+// hides behind the transforms as before (measured: late fetch there 1.68 -> 2.18 ms).
 template <int T>
-__global__ void __launch_bounds__(kThreads, T >= 8 ? 3 : 2) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
+__global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
                                                     double *__restrict__ hole, const double *__restrict__ hole_c,
                                                     const double2 *__restrict__ tw, int L, double scale0 /* -G dx0^2 */,
                                                     size_t row0, int hole_all, double *__restrict__ phi_im)
 {
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, Q = N / 4;
+    constexpr bool LATE = (T <= 8);
     using Lay = LayRow<T>;
     extern __shared__ double2 smem[];
     pdl_launch_dependents();
@@ -292,40 +296,45 @@ __global__ void __launch_bounds__(kThreads, T >= 8 ? 3 : 2) k_x_inv(const double
     const double2 *src = W1 + row * NN;
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
 
+    // a8: the prolonged contribution of the coarser levels (L2 hits: the launch before this one wrote it)
+    double ext[16];
+    auto fetch_ext = [&]() {
+        if (b > 0) {
+            pdl_wait();
+            const double *Hc = hole_c + (size_t)(b - 1) * N * N * N;
+            const int pk = Q + z / 2, pj = Q + y / 2, sk = (z & 1) ? 1 : -1, sj = (y & 1) ? 1 : -1;
+            const double *h0 = Hc + ((size_t)pk * N + pj) * N, *h1 = Hc + ((size_t)(pk + sk) * N + (pj + sj)) * N;
+#pragma unroll
+            for (int r = 0; r < 16; ++r) {
+                const int x = j + T * r, pi = Q + x / 2, si = (x & 1) ? 1 : -1;
+                ext[r] = 0.75 * __ldcg(h0 + pi) + 0.25 * __ldcg(h1 + pi + si);
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) ext[r] = 0.0;
+        }
+    };
+
+    double2 v0[16], v1[16];
+#pragma unroll
+    for (int cc = 0; cc < 16 / T; ++cc)
+#pragma unroll
+        for (int k2 = 0; k2 < T; ++k2) {
+            v0[cc * T + k2] = src[16 * k2 + cc * T + j];
+            v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
+        }
+    if (!LATE) fetch_ext();
     double2 e[16];
     {
-        double2 v0[16], v1[16], o[16];
-#pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-            for (int k2 = 0; k2 < T; ++k2) {
-                v0[cc * T + k2] = src[16 * k2 + cc * T + j];
-                v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
-            }
+        double2 o[16];
         inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
         inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncWarp());
 #pragma unroll
         for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
     }
+    if (LATE) fetch_ext();
 
-    // a8: the prolonged contribution of the coarser levels (L2 hits: the launch before this one wrote it)
     const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
-    double ext[16];
-    if (b > 0) {
-        pdl_wait();
-        const double *Hc = hole_c + (size_t)(b - 1) * N * N * N;
-        const int pk = Q + z / 2, pj = Q + y / 2, sk = (z & 1) ? 1 : -1, sj = (y & 1) ? 1 : -1;
-        const double *h0 = Hc + ((size_t)pk * N + pj) * N, *h1 = Hc + ((size_t)(pk + sk) * N + (pj + sj)) * N;
-#pragma unroll
-        for (int r = 0; r < 16; ++r) {
-            const int x = j + T * r, pi = Q + x / 2, si = (x & 1) ? 1 : -1;
-            ext[r] = 0.75 * __ldcg(h0 + pi) + 0.25 * __ldcg(h1 + pi + si);
-        }
-    } else {
-#pragma unroll
-        for (int r = 0; r < 16; ++r) ext[r] = 0.0;
-    }
-
     const double scale = scale0 * exp2(-2.0 * b);   // dx_b^2 = dx0^2 / 4^b, exact
     double *dphi = phi + row * N, *dh = hole + row * N;
 #pragma unroll
