@@ -205,25 +205,41 @@ def count_fp64_sass(kernel_substr: str):
 
 
 def ncu_row(config_id: int, kernel_substr: str):
-    """The row of the committed ncu capture profiles/r02_ncu_traffic.csv (see profiles/r02_ncu_traffic.md for the
-    command that wrote it) for this config and kernel, or None — never a hand-typed constant."""
+    """The row of the committed ncu capture for this config and kernel, or None — never a hand-typed constant.
+    profiles/r02_ncu_raw_config<id>.csv is `ncu -i <report> --page raw --csv --metrics ...` as it came out of ncu
+    (first row names, second row units; profiles/r02_ncu_raw.md holds the commands)."""
     import csv
-    path = os.path.join(ROOT, "profiles", "r02_ncu_traffic.csv")
+    path = os.path.join(ROOT, "profiles", f"r02_ncu_raw_config{config_id}.csv")
     if not os.path.exists(path):
         return None
     try:
-        for r in csv.DictReader(open(path)):
-            if int(r["config"]) == config_id and kernel_substr in r["kernel"]:
-                return r
+        rows = list(csv.reader(open(path)))
+        names, units = rows[0], rows[1]
+        for r in rows[2:]:
+            d = dict(zip(names, r))
+            if kernel_substr in d.get("Kernel Name", ""):
+                d["_units"] = dict(zip(names, units))
+                return d
     except Exception:
         pass
     return None
 
 
+_UNIT = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+
+
 def ncu_traffic(config_id: int, kernel_substr: str):
     """DRAM bytes (read + write) per launch of the kernel from that capture."""
     r = ncu_row(config_id, kernel_substr)
-    return (float(r["dram_bytes_read"]) + float(r["dram_bytes_write"])) if r else None
+    if not r:
+        return None
+    try:
+        tot = 0.0
+        for k in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+            tot += float(r[k].replace(",", "")) * _UNIT[r["_units"][k]]
+        return tot
+    except Exception:
+        return None
 
 
 # --------------------------------------------------------------------------- oracle timing (CPU)
@@ -546,9 +562,9 @@ def run_ours(args) -> None:
     kname = "k_z_conv_warp" if N == 128 else "k_z_conv_tma"
     sass = count_fp64_sass(f"{kname}ILi{T}E")
     row = ncu_row(args.config, "k_z_conv")
-    if row and row.get("fp64_warp_inst_executed"):      # executed count from the ncu capture: exact, preferred
-        per_tile = float(row["fp64_warp_inst_executed"]) * 32 / (L * (2 * N) ** 2 * T)
-        sass = {"total": per_tile, "how": "smsp__inst_executed_pipe_fp64 of the committed ncu capture / thread-tiles",
+    if row and row.get("smsp__inst_executed_pipe_fp64.sum"):      # executed count from the ncu capture: exact, preferred
+        per_tile = float(row["smsp__inst_executed_pipe_fp64.sum"].replace(",", "")) * 32 / (L * (2 * N) ** 2 * T)
+        sass = {"total": per_tile, "how": "smsp__inst_executed_pipe_fp64.sum of the committed ncu capture / thread-tiles",
                 "static_sass": sass}
     sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
     num_sms = torch.cuda.get_device_properties(dev).multi_processor_count
@@ -565,7 +581,7 @@ def run_ours(args) -> None:
     roofline["measured_limiter"] = "fp64 pipe + shared-memory pipe (on chip)" if dom == "P3_z_conv" else "hbm"
     roofline["traffic"] = ncu_traffic(args.config, {"P1_x_fwd": "k_x_fwd", "P2_y_fwd": "k_y_fwd", "P3_z_conv": "k_z_conv",
                                                     "P4_y_inv": "k_y_inv", "P5_x_inv": "k_x_inv"}[dom])
-    roofline["traffic_source"] = "profiles/r02_ncu_traffic.csv (ncu --set full capture of this kernel)" if roofline["traffic"] else None
+    roofline["traffic_source"] = f"profiles/r02_ncu_raw_config{args.config}.csv (ncu --set full capture of this kernel)" if roofline["traffic"] else None
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:

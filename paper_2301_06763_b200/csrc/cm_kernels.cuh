@@ -31,16 +31,6 @@ using cmfft::Dft;
 
 constexpr int kThreads = 128;
 
-// ---- compile-time loops over the w_32^r modulation -------------------------------
-template <int R, int DIR> struct ModW32 {
-    __device__ __forceinline__ static void run(double2 *b)
-    {
-        b[R] = cmfft::mulw32<R, DIR>(b[R]);
-        ModW32<R - 1, DIR>::run(b);
-    }
-};
-template <int DIR> struct ModW32<0, DIR> { __device__ __forceinline__ static void run(double2 *) {} };
-
 // ---- shared-memory exchange layouts ----------------------------------------------
 // One pencil's exchange buffer is a [16 (k1)][T (j)] matrix of complex, row stride RS,
 // pencil stride PS (in complex elements).  16-byte accesses: a quarter-warp (8 lanes)
@@ -109,8 +99,8 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
     double2 b[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) b[r] = a[r];
-    if (P) ModW32<15, -1>::run(b);
-    Dft<16, -1>::run(b);
+    if (P) cmfft::Dft16Mod<-1>::run(b);     // inputs times w_32^r, folded into the butterflies
+    else Dft<16, -1>::run(b);
     if (T > 1) {
         if (PRE) sync();
         double2 twp = make_double2(1.0, 0.0);
@@ -132,17 +122,27 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
     }
 }
 
-// Inverse, parity P: v as above (consumed); on return o[r] is parity P's contribution
-// to output element n = j + T r, r < 16 (the cropped half), already multiplied by
-// conj(w_32^r) for P = 1.
-template <int T, int P, class Lay, bool PRE = false, class Sync, class Tw>
-__device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm, Tw tw, Sync sync)
+// Inverse, parity P: v as above (consumed).  P = 0: on return o[r] is the even half's contribution to output
+// element n = j + T r, r < 16 (the cropped half).  P = 1: the odd half's contribution, times conj(w_32^r), is ADDED
+// to o[r] (the caller passes the even half's result).  KM: v is first multiplied by the real
+// kh[16*k2 + cc*T] (K-hat of this thread's slots, Eq. 11), folded into the first butterflies.
+template <int T, int P, class Lay, bool PRE = false, bool KM = false, class Sync, class Tw>
+__device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm, Tw tw, Sync sync,
+                                         const double *kh = nullptr)
 {
+    double2 w[16];
     if (T > 1) {
         if (PRE) sync();
 #pragma unroll
         for (int cc = 0; cc < 16 / T; ++cc) {
-            Dft<T, +1>::run(&v[cc * T]);
+            if (KM) {
+                double k[T];
+#pragma unroll
+                for (int k2 = 0; k2 < T; ++k2) k[k2] = kh[16 * k2 + cc * T];
+                cmfft::DftK<T, +1>::run(&v[cc * T], k);
+            } else {
+                Dft<T, +1>::run(&v[cc * T]);
+            }
 #pragma unroll
             for (int jj = 0; jj < T; ++jj) sm[(cc * T + j) * Lay::RS + jj] = v[cc * T + jj];
         }
@@ -150,15 +150,23 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
         double2 twp = make_double2(1.0, 0.0);
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
-            o[k1] = sm[k1 * Lay::RS + j];
-            if (k1 > 0 || P) o[k1] = cmulc(o[k1], tw_next<P>(tw, k1, twp));
+            w[k1] = sm[k1 * Lay::RS + j];
+            if (k1 > 0 || P) w[k1] = cmulc(w[k1], tw_next<P>(tw, k1, twp));
         }
     } else {
 #pragma unroll
-        for (int k1 = 0; k1 < 16; ++k1) o[k1] = v[k1];
+        for (int k1 = 0; k1 < 16; ++k1) {
+            w[k1] = v[k1];
+            if (KM) { w[k1].x *= kh[k1]; w[k1].y *= kh[k1]; }
+        }
     }
-    Dft<16, +1>::run(o);
-    if (P) ModW32<15, +1>::run(o);
+    if (P) {
+        cmfft::Dft16ModAcc<+1>::run(w, o);
+    } else {
+        Dft<16, +1>::run(w);
+#pragma unroll
+        for (int r = 0; r < 16; ++r) o[r] = w[r];
+    }
 }
 
 __device__ __forceinline__ bool in_cavity1(int v, int N) { return v >= N / 4 && v < 3 * N / 4; }
@@ -325,13 +333,8 @@ __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double
         }
     if (!LATE) fetch_ext();
     double2 e[16];
-    {
-        double2 o[16];
-        inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
-        inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncWarp());
-#pragma unroll
-        for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
-    }
+    inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
+    inv_half<T, 1, Lay>(v1, e, j, bufB, TwGlobal{tw, j}, SyncWarp());     // adds the odd half
     if (LATE) fetch_ext();
 
     const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
@@ -472,11 +475,11 @@ __global__ void __launch_bounds__(kThreads, T == 16 ? 3 : 2) k_y_inv(const doubl
             v0[cc * T + k2] = src[(size_t)(16 * k2 + cc * T + j) * NN];
             v1[cc * T + k2] = src[(size_t)(N + 16 * k2 + cc * T + j) * NN];
         }
-    double2 e[16], o[16];
+    double2 e[16];
     inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncBlock());
-    inv_half<T, 1, Lay>(v1, o, j, bufB, TwGlobal{tw, j}, SyncBlock());
+    inv_half<T, 1, Lay>(v1, e, j, bufB, TwGlobal{tw, j}, SyncBlock());   // adds the odd half
 #pragma unroll
-    for (int r = 0; r < 16; ++r) dst[(size_t)(j + T * r) * NN] = cadd(e[r], o[r]);
+    for (int r = 0; r < 16; ++r) dst[(size_t)(j + T * r) * NN] = e[r];
 }
 
 // ============================ a1: restriction cascade ==============================

@@ -92,7 +92,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
     const int ngroups = NN * NN / ZConvCfg<T>::PEN;
     // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
     const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
-    const int grid = units < 2 * p->num_sms ? (int)units : 2 * p->num_sms;
+    const int grid = units < ZConvCfg<T>::CTAS * p->num_sms ? (int)units : ZConvCfg<T>::CTAS * p->num_sms;
     if constexpr (T >= 8) {
         if (p->zconv_warp) {
             k_z_conv_warp<T><<<grid, kThreads, ZWarpCfg<T>::SMEM, s>>>(p->mapWw, p->Khat, p->tw, L, ngroups, b0);

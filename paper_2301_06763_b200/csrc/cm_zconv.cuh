@@ -83,13 +83,14 @@ template <int T> struct ZConvCfg {
     static constexpr uint32_t EX_BYTES = (T > 1) ? PEN * LayRow<T>::PS * 16 : 32768;
     static_assert(EX_BYTES >= 32768, "the exchange buffer doubles as the 32 KB output stage");
     static constexpr uint32_t TW_BYTES = 32 * T * 16;
+    static constexpr int CTAS = 2;                    // per SM (registers and shared memory both)
     static constexpr uint32_t OFF_IN = 0, OFF_KH = IN_BYTES, OFF_EX = OFF_KH + KH_BYTES, OFF_TW = OFF_EX + EX_BYTES,
                               OFF_BAR = OFF_TW + TW_BYTES;
     static constexpr uint32_t SMEM = OFF_BAR + 16 + 1024;   // + slack for the manual 1024-byte alignment
 };
 
 template <int T>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, ZConvCfg<T>::CTAS)
 k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict__ Kt,
              double2 *__restrict__ W2, const double2 *__restrict__ tw, int L, int ngroups, int b0)
 {
@@ -188,36 +189,20 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
         __syncthreads();   // every thread holds its part of the tile: the stage may be refilled
         if (tid == 0 && t + 1 < ntiles) issue_in(gn, bn);
 
-        auto kmul = [&](double2(&v)[16], int P) {
-#pragma unroll
-            for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-                for (int k2 = 0; k2 < T; ++k2) {
-                    const int s = P * N + 16 * k2 + cc * T + j;
-                    const double k = kh_p[s];
-                    v[cc * T + k2].x *= k;
-                    v[cc * T + k2].y *= k;
-                }
-        };
-
         double2 e[16];
         if (t == 0 || b == 0) {   // a new group: its K-hat tile was requested during the previous group's last tile
             mbar_wait(bar_k, ph_k);
             ph_k ^= 1;
         }
         {
-            {
-                double2 v[16];
-                fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncX());
-                kmul(v, 0);
-                inv_half<T, 0, Lay, true>(v, e, j, ex_p, tws, SyncX());
-            }
-            double2 v[16], o[16];
+            double2 v[16];
+            fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncX());
+            inv_half<T, 0, Lay, true, true>(v, e, j, ex_p, tws, SyncX(), kh_p + j);            // * K-hat, even slots
+        }
+        {
+            double2 v[16];
             fwd_half<T, 1, Lay, true>(a, v, j, ex_p, tws, SyncX());
-            kmul(v, 1);
-            inv_half<T, 1, Lay, true>(v, o, j, ex_p, tws, SyncX());
-#pragma unroll
-            for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
+            inv_half<T, 1, Lay, true, true>(v, e, j, ex_p, tws, SyncX(), kh_p + N + j);        // * K-hat, odd slots; e += odd half
         }
         // stage the output tile in the (now idle) exchange buffer with the box layout of the
         // input stage, then one thread hands it to the TMA unit: full 128-byte rows to L2.
@@ -351,39 +336,31 @@ k_z_conv_warp(const __grid_constant__ CUtensorMap mapWw, const double *__restric
             mbar_wait(bar_k, ph_k);
             ph_k ^= 1;
         }
-        auto kmul = [&](double2(&v)[16], int P) {
-#pragma unroll
-            for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-                for (int k2 = 0; k2 < T; ++k2) {
-                    const double k = kh_p[P * N + 16 * k2 + cc * T + j];
-                    v[cc * T + k2].x *= k;
-                    v[cc * T + k2].y *= k;
-                }
-        };
         double2 e[16];
         {
-            {
-                double2 v[16];
-                fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncWarp());
-                kmul(v, 0);
-                inv_half<T, 0, Lay, true>(v, e, j, ex_p, tws, SyncWarp());
-            }
-            double2 v[16], o[16];
+            double2 v[16];
+            fwd_half<T, 0, Lay, true>(a, v, j, ex_p, tws, SyncWarp());
+            inv_half<T, 0, Lay, true, true>(v, e, j, ex_p, tws, SyncWarp(), kh_p + j);         // * K-hat, even slots
+        }
+        {
+            double2 v[16];
             fwd_half<T, 1, Lay, true>(a, v, j, ex_p, tws, SyncWarp());
-            kmul(v, 1);
-            if (t + 1 < ntiles && gn != g) {      // this warp is through with the group's K-hat tile
+            // * K-hat (odd slots) rides on the first butterflies of the inverse; the second __syncwarp of inv_half
+            // (after the exchange writes) is the point where this warp is through with the group's K-hat tile
+            const bool release = t + 1 < ntiles && gn != g;
+            int nsync = 0;
+            auto sync_release = [&]() {
                 __syncwarp();
-                if (lane == 0) mbar_arrive(bar_kfree);
-                if (tid == 0) {                   // warp 0 fetches the next tile once all four warps are through
-                    mbar_wait(bar_kfree, ph_kfree);
-                    ph_kfree ^= 1;
-                    issue_k(gn);
+                if (++nsync == 2 && release) {
+                    if (lane == 0) mbar_arrive(bar_kfree);
+                    if (tid == 0) {               // warp 0 fetches the next tile once all four warps are through
+                        mbar_wait(bar_kfree, ph_kfree);
+                        ph_kfree ^= 1;
+                        issue_k(gn);
+                    }
                 }
-            }
-            inv_half<T, 1, Lay, true>(v, o, j, ex_p, tws, SyncWarp());
-#pragma unroll
-            for (int r = 0; r < 16; ++r) e[r] = cadd(e[r], o[r]);
+            };
+            inv_half<T, 1, Lay, true, true>(v, e, j, ex_p, tws, sync_release, kh_p + N + j);     // e += odd half
         }
         __syncwarp();                             // the warp's exchanges are over: its region becomes the output box
 #pragma unroll

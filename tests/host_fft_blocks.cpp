@@ -26,6 +26,62 @@ static double check()
     return e;
 }
 
+// DftK: DFT of k[i] x[i]; Dft16Mod: DFT16 of x[r] w32^{DIR r}; Dft16ModAcc: acc[r] += w32^{DIR r} DFT16(x)[r]
+template <int M, int DIR>
+static double check_k()
+{
+    double2 x[M], y[M];
+    double k[M];
+    for (int i = 0; i < M; ++i) {
+        x[i] = make_double2(std::sin(0.3 + 0.9 * i * i), std::cos(1.0 + 0.37 * i));
+        k[i] = 0.5 + std::sin(2.0 + i);
+        y[i] = make_double2(k[i] * x[i].x, k[i] * x[i].y);
+    }
+    cmfft::Dft<M, DIR>::run(y);            // checked above against the naive DFT
+    cmfft::DftK<M, DIR>::run(x, k);
+    double e = 0;
+    for (int i = 0; i < M; ++i) e = std::fmax(e, std::fmax(std::fabs(x[i].x - y[i].x), std::fabs(x[i].y - y[i].y)));
+    return e;
+}
+
+template <int DIR>
+static double check_mod()
+{
+    const long double tau = 2.0L * acosl(-1.0L);
+    double2 x[16], acc[16], acc0[16], xa[16];
+    long double rr[16], ri[16];
+    for (int i = 0; i < 16; ++i) {
+        x[i] = xa[i] = make_double2(std::sin(0.1 + 0.77 * i * i), std::cos(1.5 + 0.21 * i * i));
+        acc[i] = acc0[i] = make_double2(0.25 * i - 1.0, std::sin(3.0 * i));
+    }
+    double e = 0;
+    // modulated input
+    for (int k = 0; k < 16; ++k) {
+        long double sr = 0, si = 0;
+        for (int n = 0; n < 16; ++n) {
+            const long double a = DIR * tau * (n / 32.0L + (long double)((n * k) % 16) / 16.0L);
+            sr += x[n].x * cosl(a) - x[n].y * sinl(a);
+            si += x[n].x * sinl(a) + x[n].y * cosl(a);
+        }
+        rr[k] = sr; ri[k] = si;
+    }
+    cmfft::Dft16Mod<DIR>::run(x);
+    for (int k = 0; k < 16; ++k) e = std::fmax(e, std::fmax(std::fabs(x[k].x - (double)rr[k]), std::fabs(x[k].y - (double)ri[k])));
+    // modulated output, accumulated
+    for (int k = 0; k < 16; ++k) {
+        long double sr = 0, si = 0;
+        for (int n = 0; n < 16; ++n) {
+            const long double a = DIR * tau * (k / 32.0L + (long double)((n * k) % 16) / 16.0L);
+            sr += xa[n].x * cosl(a) - xa[n].y * sinl(a);
+            si += xa[n].x * sinl(a) + xa[n].y * cosl(a);
+        }
+        rr[k] = acc0[k].x + sr; ri[k] = acc0[k].y + si;
+    }
+    cmfft::Dft16ModAcc<DIR>::run(xa, acc);
+    for (int k = 0; k < 16; ++k) e = std::fmax(e, std::fmax(std::fabs(acc[k].x - (double)rr[k]), std::fabs(acc[k].y - (double)ri[k])));
+    return e;
+}
+
 template <int M>
 static double check_w()
 {
@@ -51,6 +107,9 @@ int main()
     e = std::fmax(e, check<4, -1>());  e = std::fmax(e, check<4, 1>());
     e = std::fmax(e, check<8, -1>());  e = std::fmax(e, check<8, 1>());
     e = std::fmax(e, check<16, -1>()); e = std::fmax(e, check<16, 1>());
+    e = std::fmax(e, check_k<1, 1>());  e = std::fmax(e, check_k<2, 1>());  e = std::fmax(e, check_k<4, 1>());
+    e = std::fmax(e, check_k<8, 1>());  e = std::fmax(e, check_k<16, 1>()); e = std::fmax(e, check_k<16, -1>());
+    e = std::fmax(e, check_mod<-1>());  e = std::fmax(e, check_mod<1>());
     double ew = WLoop<40>::run();
     // slot <-> frequency is a bijection
     int bad = 0;
