@@ -45,8 +45,11 @@ enum {
 /*
  * Create a plan for `levels` nested N^3 grids.
  *   out        : receives the plan (host pointer to a host pointer).
- *   N          : cells per axis of every level; power of two, 16 <= N <= 256
- *                (N % 4 == 0 is the method's own requirement, L76).
+ *   N          : cells per axis of every level; power of two, 16 <= N <= 512
+ *                (N % 4 == 0 is the method's own requirement, L76; N < 16 and N with factors 3 or 5 are
+ *                not built: the transform is radix-16 in registers x radix-N/16 across threads).  N = 512
+ *                runs the plain P3 kernel (no TMA staging, K-hat from global memory): it exists for the
+ *                expanded grids of the modified method and is not tuned like N <= 256.
  *   levels     : number of nested grids m >= 1 (at most 32).
  *   dx0        : cell size of level 0, > 0; dx_l = dx0 / 2^l (L48).
  *   refinement : must be 2 (the paper fixes the ratio, L42).
@@ -130,7 +133,7 @@ int cm_acceleration(cm_plan *plan, const double *phi_levels, double *g_levels, v
  * and added to the potential of the coarse grid with a cavity:
  *     Phi(Omega^n) = Phi_hole^n + reduce(Phi_dbl^{n+1}) + sum_{k<n} tilde Phi_hole^k   (n not the finest)
  *     Phi(Omega^n) = Phi^n + sum_{k<n} tilde Phi_hole^k                               (the finest grid)
- * Arguments and conventions as cm_potential.  N <= 128 (the doubled grid must be a supported size);
+ * Arguments and conventions as cm_potential.  N <= 256 (the doubled grid, 2N, must be a supported size);
  * CM_EINVAL otherwise.  The first call creates the doubled-grid plan (its K-hat: 8 (2N)^3 bytes) and
  * synchronises the device once; later calls only enqueue.  Cost: one extra (2N)^3 single-level
  * convolution per pair (the paper: x4 on CPUs, x2 with GPUs, L433).
@@ -146,7 +149,7 @@ int cm_potential_modified(cm_plan *plan, const double *rho_levels, double *phi_l
  * The doubled grid of grid n+1 has a central hole where grid n+2 lives (its mass is not counted twice); the
  * quadrupled grid is grid n+2 expanded to the size of grid n ((4N)^3 cells of its own size), reduced by the mean over
  * the 4^3 cells of a coarse cell.  qdp_direct != 0 replaces the quadrupled grid by the direct summation of Eq. B.7
- * (cm_direct_sum; centre sampling instead of the cell mean).  N <= 64 (N <= 128 with qdp_direct), else CM_EINVAL.
+ * (cm_direct_sum; centre sampling instead of the cell mean).  N <= 128 (N <= 256 with qdp_direct), else CM_EINVAL.
  * Other arguments and conventions as cm_potential_modified.
  */
 int cm_potential_modified_triplets(cm_plan *plan, const double *rho_levels, double *phi_levels, int qdp_direct, void *stream);

@@ -30,6 +30,18 @@ using cmfft::cmulc;
 using cmfft::Dft;
 
 constexpr int kThreads = 128;
+// threads of a CTA in the batch-fastest mapping (8 pencils x T threads, at least 128) and pencils it covers
+template <int T> __host__ __device__ constexpr int batch_threads() { return 8 * T > kThreads ? 8 * T : kThreads; }
+template <int T> __host__ __device__ constexpr int batch_pencils() { return batch_threads<T>() / T; }
+
+// Which slot (within one parity block of N slots) register i of thread j holds after the forward radix-T stage.
+//   T <= 16: i = cc T + k2, row k1 = cc T + j            -> slot 16 k2 + k1
+//   T = 32 (N = 512): the 32-point stage is split between two threads (below): thread j = (q, c) = (j / 16, j % 16)
+//            holds the outputs k2 = 2 i + q of row k1 = c  -> slot 16 (2 i + q) + c
+template <int T> __host__ __device__ __forceinline__ constexpr int vslot(int i, int j)
+{
+    return T <= 16 ? 16 * (i % (T <= 16 ? T : 1)) + (i / (T <= 16 ? T : 1)) * T + j : 16 * (2 * i + (j >> 4)) + (j & 15);
+}
 
 // ---- shared-memory exchange layouts ----------------------------------------------
 // One pencil's exchange buffer is a [16 (k1)][T (j)] matrix of complex, row stride RS,
@@ -110,11 +122,23 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
             sm[k1 * Lay::RS + j] = b[k1];
         }
         sync();
+        if constexpr (T <= 16) {
 #pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc) {
+            for (int cc = 0; cc < 16 / T; ++cc) {
 #pragma unroll
-            for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = sm[(cc * T + j) * Lay::RS + jj];
-            Dft<T, -1>::run(&v[cc * T]);
+                for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = sm[(cc * T + j) * Lay::RS + jj];
+                Dft<T, -1>::run(&v[cc * T]);
+            }
+        } else {
+            // 32-point stage over the threads, decimated in frequency and split between two threads: thread (q, c)
+            // forms the outputs k2 = 2 m + q of row c:  X[2m+q] = sum_jj w16^{jj m} w32^{jj q} (x[jj] + (-1)^q x[jj+16])
+            static_assert(T == 32, "radix-T stage: T <= 16 or T = 32");
+            const int q = j >> 4, c = j & 15;
+            const double sg = q ? -1.0 : 1.0;
+#pragma unroll
+            for (int jj = 0; jj < 16; ++jj) v[jj] = cmfft::cfma(sg, sm[c * Lay::RS + jj + 16], sm[c * Lay::RS + jj]);
+            if (q) cmfft::Dft16Mod<-1>::run(v);
+            else Dft<16, -1>::run(v);
         }
     } else {
 #pragma unroll
@@ -133,31 +157,66 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
     double2 w[16];
     if (T > 1) {
         if (PRE) sync();
+        if constexpr (T <= 16) {
 #pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc) {
-            if (KM) {
-                double k[T];
+            for (int cc = 0; cc < 16 / T; ++cc) {
+                if (KM) {
+                    double k[T];
 #pragma unroll
-                for (int k2 = 0; k2 < T; ++k2) k[k2] = kh[16 * k2 + cc * T];
-                cmfft::DftK<T, +1>::run(&v[cc * T], k);
+                    for (int k2 = 0; k2 < T; ++k2) k[k2] = kh[vslot<T>(cc * T + k2, j)];
+                    cmfft::DftK<T, +1>::run(&v[cc * T], k);
+                } else {
+                    Dft<T, +1>::run(&v[cc * T]);
+                }
+#pragma unroll
+                for (int jj = 0; jj < T; ++jj) sm[(cc * T + j) * Lay::RS + jj] = v[cc * T + jj];
+            }
+            sync();
+        } else {
+            // the 32-point stage backwards: thread (q, c) turns its outputs k2 = 2 m + q of row c into
+            // y_q[jj] = w32^{-q jj} sum_m V[2m+q] w16^{-m jj}; the owner of column jj + 16 h then takes y_0 + (-1)^h y_1
+            const int q = j >> 4, c = j & 15;
+            double2 y[16];
+            if (q) {
+                if (KM) {
+#pragma unroll
+                    for (int m = 0; m < 16; ++m) {
+                        const double k = kh[vslot<T>(m, j)];
+                        v[m].x *= k;
+                        v[m].y *= k;
+                    }
+                }
+#pragma unroll
+                for (int m = 0; m < 16; ++m) y[m] = make_double2(0.0, 0.0);
+                cmfft::Dft16ModAcc<+1>::run(v, y);
             } else {
-                Dft<T, +1>::run(&v[cc * T]);
+                if (KM) {
+                    double k[16];
+#pragma unroll
+                    for (int m = 0; m < 16; ++m) k[m] = kh[vslot<T>(m, j)];
+                    cmfft::DftK<16, +1>::run(v, k);
+                } else {
+                    Dft<16, +1>::run(v);
+                }
+#pragma unroll
+                for (int m = 0; m < 16; ++m) y[m] = v[m];
             }
 #pragma unroll
-            for (int jj = 0; jj < T; ++jj) sm[(cc * T + j) * Lay::RS + jj] = v[cc * T + jj];
+            for (int jj = 0; jj < 16; ++jj) sm[c * Lay::RS + 16 * q + jj] = y[jj];
+            sync();
         }
-        sync();
         double2 twp = make_double2(1.0, 0.0);
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
-            w[k1] = sm[k1 * Lay::RS + j];
+            if constexpr (T <= 16) w[k1] = sm[k1 * Lay::RS + j];
+            else w[k1] = cmfft::cfma((j >> 4) ? -1.0 : 1.0, sm[k1 * Lay::RS + 16 + (j & 15)], sm[k1 * Lay::RS + (j & 15)]);
             if (k1 > 0 || P) w[k1] = cmulc(w[k1], tw_next<P>(tw, k1, twp));
         }
     } else {
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
             w[k1] = v[k1];
-            if (KM) { w[k1].x *= kh[k1]; w[k1].y *= kh[k1]; }
+            if (KM) { w[k1].x *= kh[vslot<T>(k1, j)]; w[k1].y *= kh[vslot<T>(k1, j)]; }
         }
     }
     if (P) {
@@ -205,17 +264,13 @@ __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const
         double2 v[16];
         fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncWarp());
 #pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-            for (int k2 = 0; k2 < T; ++k2) dst[16 * k2 + cc * T + j] = v[cc * T + k2];
+        for (int i = 0; i < 16; ++i) dst[vslot<T>(i, j)] = v[i];
     }
     {
         double2 v[16];
         fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, SyncWarp());
 #pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-            for (int k2 = 0; k2 < T; ++k2) dst[N + 16 * k2 + cc * T + j] = v[cc * T + k2];
+        for (int i = 0; i < 16; ++i) dst[N + vslot<T>(i, j)] = v[i];
     }
 }
 
@@ -260,9 +315,7 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_x_fwd_split(const double *_
     else fwd_half<T, 1, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncWarp());
     double2 *dst = W1 + row * NN + P * N;
 #pragma unroll
-    for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-        for (int k2 = 0; k2 < T; ++k2) dst[16 * k2 + cc * T + j] = v[cc * T + k2];
+    for (int i = 0; i < 16; ++i) dst[vslot<T>(i, j)] = v[i];
 }
 
 // ====================== P5: x inverse + a8 (prolongation, Eq. 14) ==================
@@ -325,12 +378,10 @@ __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double
 
     double2 v0[16], v1[16];
 #pragma unroll
-    for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-        for (int k2 = 0; k2 < T; ++k2) {
-            v0[cc * T + k2] = src[16 * k2 + cc * T + j];
-            v1[cc * T + k2] = src[N + 16 * k2 + cc * T + j];
-        }
+    for (int i = 0; i < 16; ++i) {
+        v0[i] = src[vslot<T>(i, j)];
+        v1[i] = src[N + vslot<T>(i, j)];
+    }
     if (!LATE) fetch_ext();
     double2 e[16];
     inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
@@ -352,7 +403,7 @@ __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double
 
 // ======================= batch-fastest mapping (y and z passes) ====================
 // tid -> px = tid & 7 (8 adjacent slots = one 128-byte segment), j = (tid >> 3) % T,
-// g = tid / (8 T).  A CTA covers 8 * G adjacent batch positions, G = 16 / T.
+// g = tid / (8 T).  A CTA covers batch_pencils<T>() adjacent batch positions (128 threads; 256 at T = 32).
 
 // ================================ P2: y forward ====================================
 // (min-blocks choices are measured: at N = 256 P2 and P4 gain 3-5 % when compiled for 3 CTAs per
@@ -364,7 +415,7 @@ __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double
 template <int T, bool COHERENT, class Sync = SyncBlock>
 __device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, const double2 *__restrict__ tw, double2 *smem)
 {
-    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     using Lay = LayBatch<T>;
     const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
     double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
@@ -376,25 +427,21 @@ __device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, con
         double2 v[16];
         fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, Sync());
 #pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-            for (int k2 = 0; k2 < T; ++k2) dst[(size_t)(16 * k2 + cc * T + j) * NN] = v[cc * T + k2];
+        for (int i = 0; i < 16; ++i) dst[(size_t)vslot<T>(i, j) * NN] = v[i];
     }
     {
         double2 v[16];
         fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, Sync());
 #pragma unroll
-        for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-            for (int k2 = 0; k2 < T; ++k2) dst[(size_t)(N + 16 * k2 + cc * T + j) * NN] = v[cc * T + k2];
+        for (int i = 0; i < 16; ++i) dst[(size_t)(N + vslot<T>(i, j)) * NN] = v[i];
     }
 }
 
 template <int T>
-__global__ void __launch_bounds__(kThreads) k_y_fwd(const double2 *__restrict__ W1, double2 *__restrict__ W2,
+__global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd(const double2 *__restrict__ W1, double2 *__restrict__ W2,
                                                     const double2 *__restrict__ tw)
 {
-    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, px = tid & 7, g = tid / (8 * T);
     const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
@@ -408,7 +455,7 @@ template <int T>
 __global__ void __launch_bounds__(kThreads, 3) k_y_fwd_occ3(const double2 *__restrict__ W1, double2 *__restrict__ W2,
                                                     const double2 *__restrict__ tw)
 {
-    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, px = tid & 7, g = tid / (8 * T);
     const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
@@ -429,7 +476,7 @@ template <int T>
 __global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *__restrict__ W1, double2 *__restrict__ W2,
                                                                  const double2 *__restrict__ tw)
 {
-    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     using Lay = LayBatch<T>;
     extern __shared__ double2 smem[];
     const int P = threadIdx.x / kThreads, tid = threadIdx.x % kThreads;
@@ -446,17 +493,15 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *
     if (P == 0) fwd_half<T, 0, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncParity{1});
     else fwd_half<T, 1, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncParity{2});
 #pragma unroll
-    for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-        for (int k2 = 0; k2 < T; ++k2) dst[(size_t)(16 * k2 + cc * T + j) * NN] = v[cc * T + k2];
+    for (int i = 0; i < 16; ++i) dst[(size_t)vslot<T>(i, j) * NN] = v[i];
 }
 
 // ================================ P4: y inverse ====================================
 template <int T>
-__global__ void __launch_bounds__(kThreads, T == 16 ? 3 : 2) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
+__global__ void __launch_bounds__(batch_threads<T>(), T == 16 ? 3 : (T == 32 ? 1 : 2)) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
                                                     const double2 *__restrict__ tw)
 {
-    constexpr int N = 16 * T, NN = 2 * N, G = 16 / T, PEN = 8 * G;
+    constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     using Lay = LayBatch<T>;
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
@@ -469,12 +514,10 @@ __global__ void __launch_bounds__(kThreads, T == 16 ? 3 : 2) k_y_inv(const doubl
 
     double2 v0[16], v1[16];
 #pragma unroll
-    for (int cc = 0; cc < 16 / T; ++cc)
-#pragma unroll
-        for (int k2 = 0; k2 < T; ++k2) {
-            v0[cc * T + k2] = src[(size_t)(16 * k2 + cc * T + j) * NN];
-            v1[cc * T + k2] = src[(size_t)(N + 16 * k2 + cc * T + j) * NN];
-        }
+    for (int i = 0; i < 16; ++i) {
+        v0[i] = src[(size_t)vslot<T>(i, j) * NN];
+        v1[i] = src[(size_t)(N + vslot<T>(i, j)) * NN];
+    }
     double2 e[16];
     inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncBlock());
     inv_half<T, 1, Lay>(v1, e, j, bufB, TwGlobal{tw, j}, SyncBlock());   // adds the odd half

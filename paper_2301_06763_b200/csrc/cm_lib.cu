@@ -68,20 +68,24 @@ bool cuda_fail(cm_plan *p, cudaError_t e, const char *what)
     } while (0)
 
 template <int T> size_t smem_row() { return sizeof(double2) * 2 * (kThreads / T) * LayRow<T>::PS; }
-template <int T> size_t smem_batch() { return sizeof(double2) * 2 * (8 * (16 / T)) * LayBatch<T>::PS; }
+template <int T> size_t smem_batch() { return sizeof(double2) * 2 * batch_pencils<T>() * LayBatch<T>::PS; }
 
 template <int T> int set_attrs(cm_plan *p)
 {
     CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_occ3<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
-    if constexpr (T >= 8)
-        CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_warp<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZWarpCfg<T>::SMEM));
+    if constexpr (T <= 16) {
+        CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_occ3<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
+        if constexpr (T >= 8)
+            CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_warp<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZWarpCfg<T>::SMEM));
+    } else {
+        CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_batch<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    }
     return CM_OK;
 }
 
@@ -89,17 +93,22 @@ template <int T> int set_attrs(cm_plan *p)
 template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
 {
     constexpr int N = 16 * T, NN = 2 * N;
-    const int ngroups = NN * NN / ZConvCfg<T>::PEN;
-    // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
-    const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
-    const int grid = units < ZConvCfg<T>::CTAS * p->num_sms ? (int)units : ZConvCfg<T>::CTAS * p->num_sms;
-    if constexpr (T >= 8) {
-        if (p->zconv_warp) {
-            k_z_conv_warp<T><<<grid, kThreads, ZWarpCfg<T>::SMEM, s>>>(p->mapWw, p->Khat, p->tw, L, ngroups, b0);
-            return;
+    if constexpr (T <= 16) {
+        const int ngroups = NN * NN / ZConvCfg<T>::PEN;
+        // N <= 64: the kernel cuts the flat (group, level) tile list into equal ranges, so up to one CTA per tile
+        const long long units = (T <= 4) ? (long long)ngroups * L : ngroups;
+        const int grid = units < ZConvCfg<T>::CTAS * p->num_sms ? (int)units : ZConvCfg<T>::CTAS * p->num_sms;
+        if constexpr (T >= 8) {
+            if (p->zconv_warp) {
+                k_z_conv_warp<T><<<grid, kThreads, ZWarpCfg<T>::SMEM, s>>>(p->mapWw, p->Khat, p->tw, L, ngroups, b0);
+                return;
+            }
         }
+        k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0);
+    } else {
+        const unsigned ngroups = (unsigned)(NN * NN / batch_pencils<T>());
+        k_z_conv_batch<T><<<ngroups * (unsigned)L, batch_threads<T>(), smem_batch<T>(), s>>>(p->Khat, p->W2, p->tw, b0);
     }
-    k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0);
 }
 
 // P5 of level b.  chained: programmatic dependent launch on the launch before it in the stream (level b-1's P5), so
@@ -128,20 +137,33 @@ void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid,
 // level b adds the prolonged hole potentials of level b-1 (k_x_inv).
 template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev)
 {
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = 8 * (16 / T);
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
     const int L = p->L;
     const size_t planes = (size_t)L * N;
     const double scale0 = -p->G * p->dx0 * p->dx0;
-    if (p->split_x && !p->dual_in) k_x_fwd_split<T><<<(unsigned)(planes * N / ROWS), 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
-    else k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
+    bool done_x = false, done_y = false;
+    if constexpr (T <= 16) {
+        if (p->split_x && !p->dual_in) {
+            k_x_fwd_split<T><<<(unsigned)(planes * N / ROWS), 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
+            done_x = true;
+        }
+    }
+    if (!done_x) k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
     if (ev) cudaEventRecord(ev[2], s);
-    if (p->split_y) k_y_fwd_split<T><<<(unsigned)(planes * NN / PEN), 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
-    else if (T == 16) k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
-    else k_y_fwd<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    if constexpr (T <= 16) {
+        if (p->split_y) {
+            k_y_fwd_split<T><<<(unsigned)(planes * NN / PEN), 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+            done_y = true;
+        } else if (T == 16) {
+            k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+            done_y = true;
+        }
+    }
+    if (!done_y) k_y_fwd<T><<<(unsigned)(planes * NN / PEN), BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     if (ev) cudaEventRecord(ev[3], s);
     launch_zconv<T>(p, s, 0, L);
     if (ev) cudaEventRecord(ev[4], s);
-    k_y_inv<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
+    k_y_inv<T><<<(unsigned)(planes * NN / PEN), BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
     if (ev) cudaEventRecord(ev[5], s);
     const size_t lrows = (size_t)N * N;
     const unsigned gl = (unsigned)((lrows + ROWS - 1) / ROWS);
@@ -157,13 +179,13 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
 // that path is bound by the host link).
 template <int T> void level_p1_to_p4(cm_plan *p, const double *rho, cudaStream_t s, int l)
 {
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = 8 * (16 / T);
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
     const size_t lrows = (size_t)N * N;
     double2 *w1 = p->W1 + (size_t)l * lrows * NN, *w2 = p->W2 + (size_t)l * N * NN * NN;
     k_x_fwd<T><<<(unsigned)(lrows / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows, nullptr);
-    k_y_fwd<T><<<(unsigned)((size_t)N * NN / PEN), kThreads, smem_batch<T>(), s>>>(w1, w2, p->tw);
+    k_y_fwd<T><<<(unsigned)((size_t)N * NN / PEN), BT, smem_batch<T>(), s>>>(w1, w2, p->tw);
     launch_zconv<T>(p, s, l, 1);
-    k_y_inv<T><<<(unsigned)((size_t)N * NN / PEN), kThreads, smem_batch<T>(), s>>>(w2, w1, p->tw);
+    k_y_inv<T><<<(unsigned)((size_t)N * NN / PEN), BT, smem_batch<T>(), s>>>(w2, w1, p->tw);
 }
 template <int T> void level_p5(cm_plan *p, double *phi, cudaStream_t s, int l)
 {
@@ -179,6 +201,7 @@ void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, 
         case 4: p5 ? level_p5<4>(p, phi, s, l) : level_p1_to_p4<4>(p, rho, s, l); break;
         case 8: p5 ? level_p5<8>(p, phi, s, l) : level_p1_to_p4<8>(p, rho, s, l); break;
         case 16: p5 ? level_p5<16>(p, phi, s, l) : level_p1_to_p4<16>(p, rho, s, l); break;
+        case 32: p5 ? level_p5<32>(p, phi, s, l) : level_p1_to_p4<32>(p, rho, s, l); break;
     }
 }
 
@@ -204,6 +227,7 @@ int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cu
         case 4: rcode = launch_passes<4>(p, rho, phi, s, ev); break;
         case 8: rcode = launch_passes<8>(p, rho, phi, s, ev); break;
         case 16: rcode = launch_passes<16>(p, rho, phi, s, ev); break;
+        case 32: rcode = launch_passes<32>(p, rho, phi, s, ev); break;
     }
     if (rcode != CM_OK) return rcode;
     // a8 (prolongation + Eq. 14 sum) ran inside P5
@@ -288,7 +312,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
     if (!out) return CM_EINVAL;
     *out = nullptr;
     if (refinement != 2) return CM_EINVAL;
-    if (N < 16 || N > 256 || (N & (N - 1)) != 0) return CM_EINVAL;
+    if (N < 16 || N > 512 || (N & (N - 1)) != 0) return CM_EINVAL;
     if (levels < 1 || levels > 32) return CM_EINVAL;
     if (!(dx0 > 0.0) || !std::isfinite(dx0)) return CM_EINVAL;
 
@@ -342,7 +366,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         if (cuda_fail(p, cudaGetDevice(&dev), "cudaGetDevice") ||
             cuda_fail(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
             rc = CM_ECUDA;
-        else rc = make_tensor_maps(p);
+        else if (N <= 256) rc = make_tensor_maps(p);   // the TMA-fed P3 (N = 512 runs k_z_conv_batch)
     }
     if (rc == CM_OK) {
         switch (p->T) {
@@ -351,6 +375,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
             case 4: rc = set_attrs<4>(p); break;
             case 8: rc = set_attrs<8>(p); break;
             case 16: rc = set_attrs<16>(p); break;
+            case 32: rc = set_attrs<32>(p); break;
         }
     }
     if (rc != CM_OK) {
@@ -634,7 +659,7 @@ int cm_potential_modified(cm_plan *p, const double *rho, double *phi, void *stre
 {
     const int rc = check_modified_args(p, rho, phi);
     if (rc != CM_OK) return rc;
-    if (p->N > 128) return CM_EINVAL;                      // the doubled grid must be a supported size
+    if (p->N > 256) return CM_EINVAL;                      // the doubled grid must be a supported size (2N <= 512)
     return modified_impl(p, rho, phi, (cudaStream_t)stream, 2, 0);
 }
 
@@ -642,7 +667,7 @@ int cm_potential_modified_triplets(cm_plan *p, const double *rho, double *phi, i
 {
     const int rc = check_modified_args(p, rho, phi);
     if (rc != CM_OK) return rc;
-    if (p->N > 128 || (!qdp_direct && p->N > 64)) return CM_EINVAL;   // 2N (and 4N) must be supported sizes
+    if (p->N > 256 || (!qdp_direct && p->N > 128)) return CM_EINVAL;   // 2N (and 4N) must be supported sizes (<= 512)
     return modified_impl(p, rho, phi, (cudaStream_t)stream, 3, qdp_direct ? 1 : 0);
 }
 

@@ -98,13 +98,30 @@ def test_n128_every_cell_against_the_oracle(L):
     print(f"PARITY cm_potential_modified {L} x 128^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))
 
 
+def test_n256_every_cell_against_the_oracle():
+    """N = 256, the size of the paper's own dipole tests (PAPER.md:L292 uses 128^3 and 256^3 grids): the doubled grid
+    is 512^3, i.e. the N' = 512 plan (k_z_conv_batch<32>, 1024-point transforms).  Every cell against
+    oracle.solve_modified (naive FFT on the 1024^3 padded mesh: 2 x 17 GB of host memory, ~25 s on 16 threads)."""
+    psutil = pytest.importorskip("psutil")
+    if psutil.virtual_memory().available < 60e9:
+        pytest.skip("the oracle's 1024^3 complex meshes need ~45 GB of host memory")
+    N, L, dx0 = 256, 2, 2.0 / 256
+    rng = np.random.default_rng(2560 + L)
+    rho = rng.random((L, N, N, N)) * (8.0 ** np.arange(L))[:, None, None, None]
+    got, orig = _gpu(rho, dx0, G=0.9)
+    ref = oracle.solve_modified(rho, dx0, G=0.9)
+    _assert_parity(got, ref)
+    errs = [float(np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(L)]
+    print(f"PARITY cm_potential_modified {L} x 256^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))
+
+
 def test_error_codes():
     import paper_2301_06763_b200 as pkg
-    plan = pkg.Plan(256, 1, 0.1)
-    a = torch.zeros(1, 256, 256, 256, dtype=torch.float64, device="cuda")
+    plan = pkg.Plan(512, 1, 0.1)
+    a = torch.zeros(1, 512, 512, 512, dtype=torch.float64, device="cuda")
     b = torch.empty_like(a)
     with pytest.raises(pkg.CMError):
-        pkg.cm_potential_modified(plan.handle, a.data_ptr(), b.data_ptr(), 0)     # N > 128
+        pkg.cm_potential_modified(plan.handle, a.data_ptr(), b.data_ptr(), 0)     # N > 256: 2N = 1024 is not built
     plan.close()
 
 
@@ -151,9 +168,25 @@ def test_triplets_with_two_levels_is_the_pair_scheme_and_size_limits():
     rho = rng.random((2, 16, 16, 16))
     got, pairs = _gpu_triplets(rho, 0.1, False)
     assert np.array_equal(got, pairs)
-    plan = pkg.Plan(128, 1, 0.1)
-    a = torch.zeros(1, 128, 128, 128, dtype=torch.float64, device="cuda")
+    plan = pkg.Plan(256, 1, 0.1)
+    a = torch.zeros(1, 256, 256, 256, dtype=torch.float64, device="cuda")
     b = torch.empty_like(a)
     with pytest.raises(pkg.CMError):
-        pkg.cm_potential_modified_triplets(plan.handle, a.data_ptr(), b.data_ptr(), 0, 0)   # 4N = 512 unsupported
+        pkg.cm_potential_modified_triplets(plan.handle, a.data_ptr(), b.data_ptr(), 0, 0)   # 4N = 1024 unsupported
     plan.close()
+
+
+def test_triplets_n128_every_cell_against_the_oracle():
+    """N = 128, the size at which the paper quotes the triplet overhead: the quadrupled grid is 512^3
+    (N' = 512 plan).  Every cell of the three levels against oracle.solve_modified_triplets."""
+    psutil = pytest.importorskip("psutil")
+    if psutil.virtual_memory().available < 60e9:
+        pytest.skip("the oracle's 1024^3 complex meshes need ~45 GB of host memory")
+    N, L, dx0 = 128, 3, 2.0 / 128
+    rng = np.random.default_rng(1283)
+    rho = rng.random((L, N, N, N)) * (8.0 ** np.arange(L))[:, None, None, None]
+    got, pairs = _gpu_triplets(rho, dx0, False, G=1.1)
+    ref = oracle.solve_modified_triplets(rho, dx0, G=1.1, qdp="fft")
+    _assert_parity(got, ref)
+    errs = [float(np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(L)]
+    print(f"PARITY cm_potential_modified_triplets {L} x 128^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))

@@ -299,7 +299,7 @@ def test_G_scales_linearly_and_error_codes():
     assert np.abs(b - 6.674e-8 * a).max() <= 1e-15 * np.abs(b).max()
     p1.close()
     p2.close()
-    for bad in [dict(N=24, levels=2, dx0=1.0), dict(N=8, levels=2, dx0=1.0), dict(N=512, levels=2, dx0=1.0),
+    for bad in [dict(N=24, levels=2, dx0=1.0), dict(N=8, levels=2, dx0=1.0), dict(N=1024, levels=2, dx0=1.0),
                 dict(N=16, levels=0, dx0=1.0), dict(N=16, levels=2, dx0=0.0), dict(N=16, levels=2, dx0=1.0, refinement=3)]:
         with pytest.raises(pkg.CMError) as ei:
             pkg.cm_plan_create(**bad)
@@ -371,3 +371,29 @@ def test_single_level_at_the_largest_grid():
     for t, r in zip(targets, ref):
         assert abs(got[t] - r) <= TOL * scale, (t, got[t], r)
     plan.close()
+
+
+def test_two_level_nest_at_512_whole_grid_and_host_entry_point():
+    """N = 512 (T = 32: the 32-point stage split between two threads, k_z_conv_batch): a 2-level random nest, every
+    cell against the FFT oracle (1024^3 complex meshes: ~35 GB of host memory, ~25 s per field on 16 threads), plus
+    sampled direct sums as an FFT-free witness, and cm_potential_host bit-identical to cm_potential."""
+    psutil = pytest.importorskip("psutil")
+    N, L = 512, 2
+    rng = np.random.default_rng(512)
+    rho = rng.random((L, N, N, N)) * (4.0 ** np.arange(L))[:, None, None, None]
+    got, plan = _solve_gpu(rho, 2.0 / N)
+    targets = [(0, 0, 0, 0), (0, 511, 511, 511), (0, 17, 400, 100), (0, 256, 255, 128), (1, 0, 0, 0), (1, 511, 3, 77),
+               (1, 255, 256, 257), (1, 1, 510, 128)]
+    pts = oracle.solve_points(rho, 2.0 / N, targets)
+    for t, r in zip(targets, pts):
+        assert abs(got[t] - r) <= TOL * np.abs(got[t[0]]).max(), (t, got[t], r)
+    host = plan.potential_host(torch.from_numpy(rho).pin_memory())
+    torch.cuda.synchronize()
+    assert np.array_equal(host.numpy(), got)
+    plan.close()
+    if psutil.virtual_memory().available < 60e9:
+        pytest.skip("whole-grid part skipped: the oracle's 1024^3 complex meshes need ~45 GB of host memory")
+    ref = oracle.solve(rho, 2.0 / N, method="fft")
+    _assert_parity(got, ref)
+    errs = [float(np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(L)]
+    print("PARITY 2 x 512^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))
