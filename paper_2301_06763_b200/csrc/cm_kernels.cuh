@@ -71,33 +71,37 @@ struct TwGlobal {
     int j;
     static constexpr bool RECUR = false;
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return __ldg(&tw[j * (2 * k1 + P)]); }
-    __device__ __forceinline__ double2 step() const { return make_double2(1.0, 0.0); }
-    __device__ __forceinline__ double2 step2() const { return make_double2(1.0, 0.0); }
-    __device__ __forceinline__ double2 step3() const { return make_double2(1.0, 0.0); }
 };
-// P3 is bound by the shared-memory data pipe (profiles/r01b), not by fp64: only every fourth twiddle (k1 = 0, 4,
-// 8, 12) is read from the table; the three after it are that one times rho, rho^2, rho^3 (rho = w_2N^{2j}, the
-// powers kept in registers; one extra rounding, ~1e-16).
+// P3 is bound by the shared-memory data pipe as much as by fp64 (profiles/): only every fourth twiddle (k1 = 0, 4, 8,
+// 12) is read from the table.  The ones between follow from the three-term recurrence of a geometric sequence,
+//     t[k+1] = 2 cos(phi) t[k] - t[k-1],   phi = arg of the ratio rho = w_2N^{2 j},
+// one FMA per component (a complex multiply by rho would be four); an anchor from the table every fourth step keeps
+// the rounding error at a few ulp (the recurrence amplifies it quadratically in the step count only).
 template <int T> struct TwShared {
     const double2 *base;   // table + j
     double2 rho;           // w_2N^{2 j}
-    double2 rho2, rho3;    // w_2N^{4 j}, w_2N^{6 j}
     static constexpr bool RECUR = true;
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return base[(2 * k1 + P) * T]; }
-    __device__ __forceinline__ double2 step() const { return rho; }
-    __device__ __forceinline__ double2 step2() const { return rho2; }
-    __device__ __forceinline__ double2 step3() const { return rho3; }
 };
 
-// twiddle w_2N^{j (2 k1 + P)} for k1 = 0..15 in turn; `prev` carries the last value read from the table
-template <int P, class Tw> __device__ __forceinline__ double2 tw_next(const Tw &tw, int k1, double2 &prev)
+// twiddle w_2N^{j (2 k1 + P)} for k1 = 0..15 in turn; p1 / p2 carry the two values before it
+struct TwCarry { double2 p1, p2; };
+template <int P, class Tw> __device__ __forceinline__ double2 tw_next(const Tw &tw, int k1, TwCarry &c)
 {
-    if (Tw::RECUR && (k1 & 3)) {
-        const double2 r = (k1 & 3) == 1 ? tw.step() : ((k1 & 3) == 2 ? tw.step2() : tw.step3());
-        return (P == 0 && k1 < 4) ? r : cmul(prev, r);
+    double2 t;
+    if constexpr (Tw::RECUR) {
+        if ((k1 & 3) == 0) t = (P == 0 && k1 == 0) ? make_double2(1.0, 0.0) : tw.template get<P>(k1);
+        else if (k1 == 1) t = (P == 0) ? tw.rho : cmul(c.p1, tw.rho);
+        else {
+            const double c2 = 2.0 * tw.rho.x;
+            t = make_double2(fma(c2, c.p1.x, -c.p2.x), fma(c2, c.p1.y, -c.p2.y));
+        }
+    } else {
+        t = tw.template get<P>(k1);
     }
-    prev = tw.template get<P>(k1);
-    return prev;
+    c.p2 = c.p1;
+    c.p1 = t;
+    return t;
 }
 
 // ---- half transforms ---------------------------------------------------------------
@@ -115,10 +119,11 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
     else Dft<16, -1>::run(b);
     if (T > 1) {
         if (PRE) sync();
-        double2 twp = make_double2(1.0, 0.0);
+        TwCarry twc{make_double2(1.0, 0.0), make_double2(1.0, 0.0)};
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
-            if (k1 > 0 || P) b[k1] = cmul(b[k1], tw_next<P>(tw, k1, twp));
+            const double2 t = tw_next<P>(tw, k1, twc);
+            if (k1 > 0 || P) b[k1] = cmul(b[k1], t);
             sm[k1 * Lay::RS + j] = b[k1];
         }
         sync();
@@ -150,10 +155,13 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
 // element n = j + T r, r < 16 (the cropped half).  P = 1: the odd half's contribution, times conj(w_32^r), is ADDED
 // to o[r] (the caller passes the even half's result).  KM: v is first multiplied by the real
 // kh[16*k2 + cc*T] (K-hat of this thread's slots, Eq. 11), folded into the first butterflies.
-template <int T, int P, class Lay, bool PRE = false, bool KM = false, class Sync, class Tw>
+// DEC > 1 (cm_expand.cuh): only the threads with j % DEC == 0 run the last stage — their outputs n = j + T r are the
+// multiples of DEC, all a decimated inverse keeps; the others only take part in the exchange.
+template <int T, int P, class Lay, bool PRE = false, bool KM = false, int DEC = 1, class Sync, class Tw>
 __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm, Tw tw, Sync sync,
                                          const double *kh = nullptr)
 {
+    static_assert(DEC == 1 || (T > 1 && T % DEC == 0), "decimation needs the radix-T stage");
     double2 w[16];
     if (T > 1) {
         if (PRE) sync();
@@ -205,12 +213,14 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
             for (int jj = 0; jj < 16; ++jj) sm[c * Lay::RS + 16 * q + jj] = y[jj];
             sync();
         }
-        double2 twp = make_double2(1.0, 0.0);
+        if (DEC > 1 && (j % DEC) != 0) return;
+        TwCarry twc{make_double2(1.0, 0.0), make_double2(1.0, 0.0)};
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
             if constexpr (T <= 16) w[k1] = sm[k1 * Lay::RS + j];
             else w[k1] = cmfft::cfma((j >> 4) ? -1.0 : 1.0, sm[k1 * Lay::RS + 16 + (j & 15)], sm[k1 * Lay::RS + (j & 15)]);
-            if (k1 > 0 || P) w[k1] = cmulc(w[k1], tw_next<P>(tw, k1, twp));
+            const double2 t = tw_next<P>(tw, k1, twc);
+            if (k1 > 0 || P) w[k1] = cmulc(w[k1], t);
         }
     } else {
 #pragma unroll
@@ -237,8 +247,7 @@ __device__ __forceinline__ bool in_ring1(int v, int N) { return v >= N / 4 - 1 &
 // body: thread (rowl, j) of a CTA transforms global row `row` (b, z, y) and writes its 2N slots to `dst`
 template <int T>
 __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const double *__restrict__ rc, double2 *dst,
-                                           const double2 *__restrict__ tw, int L, size_t row, double2 *smem,
-                                           const double *__restrict__ rho_im = nullptr)
+                                           const double2 *__restrict__ tw, int L, size_t row, double2 *smem)
 {
     constexpr int N = 16 * T, ROWS = kThreads / T, H = N / 2, Q = N / 4;
     using Lay = LayRow<T>;
@@ -255,9 +264,7 @@ __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const
         const int x = j + T * r;
         const bool cav = rowcav && in_cavity1(x, N);
         const double re = cav ? __ldg(srcc + x) : __ldg(src + x);
-        // rho_im (single-level plans only): a second, independent real field rides as the imaginary part —
-        // K-hat is real, so its potential comes out as the imaginary part of the result (cm_potential_modified)
-        a[r] = make_double2(re, rho_im ? __ldg(rho_im + row * N + x) : ((finest || cav) ? 0.0 : re));
+        a[r] = make_double2(re, (finest || cav) ? 0.0 : re);
     }
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
     {
@@ -277,13 +284,13 @@ __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const
 template <int T>
 __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ rho, const double *__restrict__ rc,
                                                     double2 *__restrict__ W1, const double2 *__restrict__ tw, int L,
-                                                    size_t row0, const double *__restrict__ rho_im)
+                                                    size_t row0)
 {
     // row0: first global row (b, z, y) of this launch
     constexpr int NN = 32 * T, ROWS = kThreads / T;
     extern __shared__ double2 smem[];
     const size_t row = row0 + (size_t)blockIdx.x * ROWS + threadIdx.x / T;
-    x_fwd_body<T>(rho, rc, W1 + row * NN, tw, L, row, smem, rho_im);
+    x_fwd_body<T>(rho, rc, W1 + row * NN, tw, L, row, smem);
 }
 
 // P1 split by output parity (see k_y_fwd_split): 256 threads, warps 0-3 the even slots, warps 4-7 the odd ones
@@ -344,7 +351,7 @@ template <int T>
 __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
                                                     double *__restrict__ hole, const double *__restrict__ hole_c,
                                                     const double2 *__restrict__ tw, int L, double scale0 /* -G dx0^2 */,
-                                                    size_t row0, int hole_all, double *__restrict__ phi_im)
+                                                    size_t row0, int hole_all)
 {
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, Q = N / 4;
     constexpr bool LATE = (T <= 8);
@@ -397,7 +404,6 @@ __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double
         const double re = scale * e[r].x, im = scale * e[r].y;
         dphi[x] = b > 0 ? re + ext[r] : re;
         if (hole_all ? (b < L - 1) : (rowring && in_ring1(x, N))) dh[x] = b > 0 ? im + ext[r] : im;
-        if (phi_im) phi_im[row * N + x] = im;       // the second field of a dual single-level solve
     }
 }
 
@@ -410,10 +416,11 @@ __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double
 // SM (168 registers); at smaller N P2 is best left to ptxas (178 registers) and P4 with a floor of 2 CTAs,
 // which lets ptxas use 230 registers: -15 % at N = 128)
 // body: the CTA transforms PEN = 8 * (16/T) adjacent sx columns of one (b, z) plane; src/dst point at
-// this thread's column (sx) of the plane's W1 rows / W2 rows.  COHERENT: read W1 through L2 only
-// (ld.global.cg) — needed when another CTA of the same kernel produced it (cm_fused.cuh).
-template <int T, bool COHERENT, class Sync = SyncBlock>
-__device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, const double2 *__restrict__ tw, double2 *smem)
+// this thread's column (sx) of the plane's W1 rows / W2 rows.  [ylo, yhi): the rows that hold data (the rest of the
+// column is taken as zero without being read: the expanded grids of cm_expand.cuh); the whole column by default.
+template <int T, class Sync = SyncBlock>
+__device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, const double2 *__restrict__ tw, double2 *smem,
+                                           int ylo = 0, int yhi = 16 * T)
 {
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     using Lay = LayBatch<T>;
@@ -422,7 +429,10 @@ __device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, con
 
     double2 a[16];
 #pragma unroll
-    for (int r = 0; r < 16; ++r) a[r] = COHERENT ? __ldcg(src + (size_t)(j + T * r) * NN) : src[(size_t)(j + T * r) * NN];
+    for (int r = 0; r < 16; ++r) {
+        const int y = j + T * r;
+        a[r] = (y >= ylo && y < yhi) ? src[(size_t)y * NN] : make_double2(0.0, 0.0);
+    }
     {
         double2 v[16];
         fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, Sync());
@@ -447,7 +457,7 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd(const double2 *__r
     const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
-    y_fwd_body<T, false>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
+    y_fwd_body<T>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
 }
 
 // the same kernel compiled for 3 CTAs per SM (168 registers): used at N = 256
@@ -461,7 +471,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_y_fwd_occ3(const double2 *__res
     const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
-    y_fwd_body<T, false>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
+    y_fwd_body<T>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
 }
 
 // P2 split by output parity: 256 threads, warps 0-3 form the even slots (P = 0), warps 4-7 the odd ones

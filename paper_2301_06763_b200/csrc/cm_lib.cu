@@ -11,6 +11,7 @@
 #include "../../include/cm.h"
 #include "cm_kernels.cuh"
 #include "cm_zconv.cuh"
+#include "cm_expand.cuh"
 
 namespace {
 
@@ -37,8 +38,7 @@ struct cm_plan {
     cm_plan *dbl = nullptr, *qdp = nullptr;   // single-level plans of the doubled (2N)^3 and quadrupled (4N)^3 fine grid
     double *rho4 = nullptr, *phi4 = nullptr, *tmp3 = nullptr;
     double *rho2 = nullptr, *phi2 = nullptr;   // two doubled grids each: one complex solve serves two pairs
-    const double *dual_in = nullptr;            // single-level plans: second real field in / its potential out
-    double *dual_out = nullptr;
+    double2 *decE = nullptr;                    // expanded-grid plans: E(k) of the decimated inverse, slot order (cm_expand.cuh)
     bool use_graph = true;
     cudaStream_t cap_stream = nullptr, copy_stream = nullptr;
     std::vector<cudaEvent_t> ev_level;   // cm_potential_host's pipeline: [0,32) level arrived, [32,64) level's Phi ready, [64] start
@@ -115,7 +115,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
 // that this level's loads and transforms overlap that level's tail; the kernel waits (griddepcontrol.wait) only
 // before it reads what level b-1 wrote.
 template <int T>
-void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid, double scale0, double *phi_im, bool chained)
+void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid, double scale0, bool chained)
 {
     constexpr int N = 16 * T;
     cudaLaunchConfig_t cfg = {};
@@ -129,7 +129,7 @@ void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid,
     cfg.attrs = at;
     cfg.numAttrs = chained ? 1 : 0;
     cudaLaunchKernelEx(&cfg, k_x_inv<T>, (const double2 *)p->W1, phi, p->hole, (const double *)p->hole, (const double2 *)p->tw, p->L,
-                       scale0, (size_t)b * N * N, p->hole_all, phi_im);
+                       scale0, (size_t)b * N * N, p->hole_all);
 }
 
 // The five FFT passes (steps a3-a7) with the prolongation + Eq. 14 sum (a8) folded into P5:
@@ -143,12 +143,12 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     const double scale0 = -p->G * p->dx0 * p->dx0;
     bool done_x = false, done_y = false;
     if constexpr (T <= 16) {
-        if (p->split_x && !p->dual_in) {
+        if (p->split_x) {
             k_x_fwd_split<T><<<(unsigned)(planes * N / ROWS), 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
             done_x = true;
         }
     }
-    if (!done_x) k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, p->dual_in);
+    if (!done_x) k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
     if (ev) cudaEventRecord(ev[2], s);
     if constexpr (T <= 16) {
         if (p->split_y) {
@@ -167,7 +167,7 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     if (ev) cudaEventRecord(ev[5], s);
     const size_t lrows = (size_t)N * N;
     const unsigned gl = (unsigned)((lrows + ROWS - 1) / ROWS);
-    for (int b = 0; b < L; ++b) launch_x_inv<T>(p, phi, s, b, gl, scale0, p->dual_out, /*chained=*/b > 0);
+    for (int b = 0; b < L; ++b) launch_x_inv<T>(p, phi, s, b, gl, scale0, /*chained=*/b > 0);
     if (ev) cudaEventRecord(ev[6], s);
     p->launches += 4 + L;
     CM_CUDA(p, cudaGetLastError());
@@ -182,7 +182,7 @@ template <int T> void level_p1_to_p4(cm_plan *p, const double *rho, cudaStream_t
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
     const size_t lrows = (size_t)N * N;
     double2 *w1 = p->W1 + (size_t)l * lrows * NN, *w2 = p->W2 + (size_t)l * N * NN * NN;
-    k_x_fwd<T><<<(unsigned)(lrows / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows, nullptr);
+    k_x_fwd<T><<<(unsigned)(lrows / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows);
     k_y_fwd<T><<<(unsigned)((size_t)N * NN / PEN), BT, smem_batch<T>(), s>>>(w1, w2, p->tw);
     launch_zconv<T>(p, s, l, 1);
     k_y_inv<T><<<(unsigned)((size_t)N * NN / PEN), BT, smem_batch<T>(), s>>>(w2, w1, p->tw);
@@ -191,7 +191,7 @@ template <int T> void level_p5(cm_plan *p, double *phi, cudaStream_t s, int l)
 {
     constexpr int N = 16 * T, ROWS = kThreads / T;
     const size_t lrows = (size_t)N * N;
-    launch_x_inv<T>(p, phi, s, l, (unsigned)((lrows + ROWS - 1) / ROWS), -p->G * p->dx0 * p->dx0, nullptr, /*chained=*/false);
+    launch_x_inv<T>(p, phi, s, l, (unsigned)((lrows + ROWS - 1) / ROWS), -p->G * p->dx0 * p->dx0, /*chained=*/false);
 }
 void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int l, bool p5)
 {
@@ -544,25 +544,82 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
 
 namespace {
 
-// one expanded-grid plan (N' = F N, one level, unit G and dx) with room for two fields (dual solve)
-int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **rho_big, double **phi_big)
+// The five passes of an expanded-grid solve (cm_expand.cuh) on the single-level plan pe of size N' = 16 T = F Nc:
+// forward passes pruned to the central Nc^3 block, inverse passes decimated by F.  src_re / src_im: compact Nc^3
+// densities (src_im optional: the second real field); out_re / out_im: minus the block SUMS of their potentials.
+template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, const double *src_im, double *out_re, double *out_im,
+                                            cudaStream_t s)
 {
-    if (*plan && *rho_big && *phi_big) return CM_OK;
-    const size_t n3 = (size_t)p->N * p->N * p->N, big = (size_t)F * F * F * n3;
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>(), Nc = N / F,
+                  c0 = (N - Nc) / 2;
+    static bool attrs = false;      // per instantiation; the attribute is per function, not per plan
+    if (!attrs) {
+        CM_CUDA(pe, cudaFuncSetAttribute(k_x_fwd_blk<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+        CM_CUDA(pe, cudaFuncSetAttribute(k_y_fwd_blk<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(pe, cudaFuncSetAttribute(k_z_conv_dec<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZDecCfg<T>::SMEM));
+        CM_CUDA(pe, cudaFuncSetAttribute(k_y_inv_dec<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(pe, cudaFuncSetAttribute(k_x_inv_dec<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+        attrs = true;
+    }
+    k_x_fwd_blk<T><<<(unsigned)(Nc * Nc / ROWS), kThreads, smem_row<T>(), s>>>(src_re, src_im, pe->W1, pe->tw, Nc, c0);
+    k_y_fwd_blk<T><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W1, pe->W2, pe->tw, Nc, c0);
+    k_z_conv_dec<T, F><<<(unsigned)((size_t)(N + 1) * (NN / PEN)), BT, ZDecCfg<T>::SMEM, s>>>(pe->Khat, pe->W2, pe->tw, pe->decE, c0, c0 + Nc);
+    k_y_inv_dec<T, F><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W2, pe->W1, pe->tw, pe->decE);
+    k_x_inv_dec<T, F><<<(unsigned)(Nc * Nc / ROWS), kThreads, smem_row<T>(), s>>>(pe->W1, out_re, out_im, pe->tw, pe->decE, -1.0);
+    CM_CUDA(pe, cudaGetLastError());
+    return CM_OK;
+}
+
+int dispatch_expanded(cm_plan *pe, int F, const double *src_re, const double *src_im, double *out_re, double *out_im, cudaStream_t s)
+{
+#define CM_EXP(TT, FF) \
+    if (pe->T == TT && F == FF) return expanded_passes<TT, FF>(pe, src_re, src_im, out_re, out_im, s);
+    CM_EXP(2, 2) CM_EXP(4, 2) CM_EXP(8, 2) CM_EXP(16, 2) CM_EXP(32, 2)
+    CM_EXP(4, 4) CM_EXP(8, 4) CM_EXP(16, 4) CM_EXP(32, 4)
+#undef CM_EXP
+    return CM_EINVAL;
+}
+
+// one expanded-grid plan (N' = F N, one level, unit G and dx: it supplies K-hat, the twiddles and W1 / W2), the table
+// E(k) = sum_{q<F} e^{2 pi i k q / 2N'} in slot order, and compact N^3 buffers for two sources and two results
+int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **src, double **res)
+{
+    if (*plan && *src && *res) return CM_OK;
+    const size_t n3 = (size_t)p->N * p->N * p->N;
     const size_t keep = p->bytes;
     int rc = CM_OK;
     if (!*plan) rc = cm_plan_create(plan, F * p->N, 1, 1.0, 2);
     if (rc == CM_OK) rc = cm_green_precompute(*plan);
-    if (rc == CM_OK && !*rho_big) rc = dev_alloc(p, rho_big, 2 * big);
-    if (rc == CM_OK && !*phi_big) rc = dev_alloc(p, phi_big, 2 * big);
+    if (rc == CM_OK && !(*plan)->decE) {
+        cm_plan *pe = *plan;
+        const int n = 2 * pe->N;
+        rc = dev_alloc(pe, &pe->decE, (size_t)n);
+        if (rc == CM_OK) {
+            std::vector<double2> E(n);
+            const long double tau = 2.0L * acosl(-1.0L);
+            for (int sl = 0; sl < n; ++sl) {
+                const int k = cmfft::slot_to_freq(sl, pe->N);
+                long double re = 0, im = 0;
+                for (int q = 0; q < F; ++q) {
+                    const long double a = tau * (long double)(((long long)k * q) % n) / (long double)n;
+                    re += cosl(a);
+                    im += sinl(a);
+                }
+                E[sl] = make_double2((double)re, (double)im);
+            }
+            if (cuda_fail(p, cudaMemcpy(pe->decE, E.data(), n * sizeof(double2), cudaMemcpyHostToDevice), "cudaMemcpy(E)")) rc = CM_ECUDA;
+        }
+    }
+    if (rc == CM_OK && !*src) rc = dev_alloc(p, src, 2 * n3);
+    if (rc == CM_OK && !*res) rc = dev_alloc(p, res, 2 * n3);
     if (rc != CM_OK) {
         // all or nothing: a later call must not find a half-built expanded plan
         if (*plan) std::snprintf(p->err, sizeof(p->err), "expanded-grid plan (x%d): %.400s", F, (*plan)->err);
         cm_plan_destroy(*plan);
         *plan = nullptr;
-        cudaFree(*rho_big);
-        cudaFree(*phi_big);
-        *rho_big = *phi_big = nullptr;
+        cudaFree(*src);
+        cudaFree(*res);
+        *src = *res = nullptr;
         p->bytes = keep;
         return rc;
     }
@@ -570,21 +627,17 @@ int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **rho_big, double 
     return CM_OK;
 }
 
-// Expanded grids of levels l1 and (optionally) l1b through ONE complex single-level solve (K-hat is real: the second
-// density rides as the imaginary part); results -(rho * g) in phi_big and phi_big + big.
-int solve_expanded(cm_plan *p, cm_plan *pe, int F, const double *rho, double *rho_big, double *phi_big, cudaStream_t s, int l1,
-                   int hole1, int l1b, int hole1b)
+// Expanded grids of levels l1 and (optionally) l1b through ONE complex solve (K-hat real, E Hermitian: the second
+// density rides as the imaginary part); res and res + N^3 receive minus the block sums of rho * g over the F^3 cells
+// of a coarse cell.
+int solve_expanded(cm_plan *p, cm_plan *pe, int F, const double *rho, double *src, double *res, cudaStream_t s, int l1, int hole1,
+                   int l1b, int hole1b)
 {
-    const size_t n3 = (size_t)p->N * p->N * p->N, big = (size_t)F * F * F * n3;
-    const unsigned g = (unsigned)((big + 255) / 256);
-    k_pad_expand<<<g, 256, 0, s>>>(p->N, F, hole1, l1, p->L, rho, p->rc, rho_big);
-    if (l1b >= 0) k_pad_expand<<<g, 256, 0, s>>>(p->N, F, hole1b, l1b, p->L, rho, p->rc, rho_big + big);
-    pe->dual_in = l1b >= 0 ? rho_big + big : nullptr;
-    pe->dual_out = l1b >= 0 ? phi_big + big : nullptr;
-    const int rc = enqueue_solve(pe, rho_big, phi_big, s);
-    pe->dual_in = nullptr;
-    pe->dual_out = nullptr;
-    return rc;
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    const unsigned g = (unsigned)((n3 + 255) / 256);
+    k_pad_expand<<<g, 256, 0, s>>>(p->N, 1, hole1, l1, p->L, rho, p->rc, src);          // rho-bar of grid l1 (optionally holed)
+    if (l1b >= 0) k_pad_expand<<<g, 256, 0, s>>>(p->N, 1, hole1b, l1b, p->L, rho, p->rc, src + n3);
+    return dispatch_expanded(pe, F, src, l1b >= 0 ? src + n3 : nullptr, res, l1b >= 0 ? res + n3 : nullptr, s);
 }
 
 int direct_sum_impl(cm_plan *p, const double *rho_src, int src_level, int dst_level, double *phi_dst, cudaStream_t s);
@@ -607,7 +660,6 @@ int modified_impl(cm_plan *p, const double *rho, double *phi, cudaStream_t s, in
     if (rc != CM_OK) return rc;
     // doubled grids: Phi(Omega^n) = H_n + reduce(Phi_dbl^{n+1}), two pairs per complex solve; in the triplet scheme the
     // doubled grid has a central hole (grid n+2's mass comes through the quadrupled grid) except for the last pair (B.5)
-    const size_t d3 = 8 * n3, q3 = 64 * n3;
     for (int n = 0; n + 1 < L; n += 2) {
         const bool two = n + 2 < L;
         const int h0 = triple && n < L - 2, h1 = triple && n + 1 < L - 2;
@@ -615,7 +667,7 @@ int modified_impl(cm_plan *p, const double *rho, double *phi, cudaStream_t s, in
         if (rc != CM_OK) return rc;
         for (int q = 0; q < (two ? 2 : 1); ++q) {
             const double dxf = p->dx0 * std::exp2(-(double)(n + q + 1));
-            k_add_block_mean<<<gn, 256, 0, s>>>(N, 2, p->hole + (n + q) * n3, p->phi2 + q * d3, p->G * dxf * dxf, phi + (n + q) * n3);
+            k_add_block_mean<<<gn, 256, 0, s>>>(N, 1, p->hole + (n + q) * n3, p->phi2 + q * n3, p->G * dxf * dxf / 8.0, phi + (n + q) * n3);
         }
     }
     // quadrupled grids (B.3): + reduce(Phi_qdp^{n+2}) for n < L-2, by the same convolution or by direct summation (B.7)
@@ -632,7 +684,7 @@ int modified_impl(cm_plan *p, const double *rho, double *phi, cudaStream_t s, in
                 if (rc != CM_OK) return rc;
                 for (int q = 0; q < (two ? 2 : 1); ++q) {
                     const double dxf = p->dx0 * std::exp2(-(double)(n + q + 2));
-                    k_add_block_mean<<<gn, 256, 0, s>>>(N, 4, phi + (n + q) * n3, p->phi4 + q * q3, p->G * dxf * dxf, phi + (n + q) * n3);
+                    k_add_block_mean<<<gn, 256, 0, s>>>(N, 1, phi + (n + q) * n3, p->phi4 + q * n3, p->G * dxf * dxf / 64.0, phi + (n + q) * n3);
                 }
             }
         }
@@ -745,6 +797,7 @@ int cm_plan_destroy(cm_plan *p)
     cudaFree(p->phi4);
     cudaFree(p->tmp3);
     cudaFree(p->tw);
+    cudaFree(p->decE);
     cudaFree(p->stage_rho);
     cudaFree(p->stage_phi);
     delete p;

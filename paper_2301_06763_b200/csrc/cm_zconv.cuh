@@ -169,7 +169,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
     const unsigned char *in_p = sbase + C::OFF_IN + bx * (N * 128);
     const double *kh_p = reinterpret_cast<const double *>(sbase + C::OFF_KH) + pen * C::RSK;
     double2 *ex_p = ex_s + pen * Lay::PS;
-    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j], tw_s[4 * T + j], tw_s[6 * T + j]};
+    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j]};
     using SyncX = SyncWarp;
     uint32_t ph_in = 0, ph_k = 0;
 
@@ -311,7 +311,7 @@ k_z_conv_warp(const __grid_constant__ CUtensorMap mapWw, const double *__restric
         if (lane == 0) issue_in(g0, bb0);
     }
     const double *kh_p = reinterpret_cast<const double *>(sbase + W::OFF_KH) + pen * C::RSK;
-    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j], tw_s[4 * T + j], tw_s[6 * T + j]};
+    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j]};
     // swizzled position of (row z, pencil pxl) in a warp's box: 32B rows: chunk bit0 ^= bit 7 of the offset;
     // 64B rows: chunk bits [1:0] ^= bits [8:7]
     auto box_off = [&](int z) -> uint32_t {
