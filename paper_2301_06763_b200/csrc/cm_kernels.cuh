@@ -348,7 +348,7 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 // N = 256 (a level is 28 waves, the overlap is worth little): wait first and fetch Hc at the top, so that its latency
 // hides behind the transforms as before (measured: late fetch there 1.68 -> 2.18 ms).
 template <int T>
-__global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
+__global__ void __launch_bounds__(kThreads, 2) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
                                                     double *__restrict__ hole, const double *__restrict__ hole_c,
                                                     const double2 *__restrict__ tw, int L, double scale0 /* -G dx0^2 */,
                                                     size_t row0, int hole_all)
@@ -412,9 +412,9 @@ __global__ void __launch_bounds__(kThreads, T == 8 ? 3 : 2) k_x_inv(const double
 // g = tid / (8 T).  A CTA covers batch_pencils<T>() adjacent batch positions (128 threads; 256 at T = 32).
 
 // ================================ P2: y forward ====================================
-// (min-blocks choices are measured: at N = 256 P2 and P4 gain 3-5 % when compiled for 3 CTAs per
-// SM (168 registers); at smaller N P2 is best left to ptxas (178 registers) and P4 with a floor of 2 CTAs,
-// which lets ptxas use 230 registers: -15 % at N = 128)
+// (min-blocks choices are measured, DESIGN.md §6 / profiles/r02_pass_variants.md: with the FMA-fused butterflies every
+// pass is best with a floor of 2 CTAs per SM, which lets ptxas use up to 255 registers — capping P4 or P5 at 168
+// registers for a third CTA costs 25-45 %; P2 at N <= 128 is left to ptxas (178 registers))
 // body: the CTA transforms PEN = 8 * (16/T) adjacent sx columns of one (b, z) plane; src/dst point at
 // this thread's column (sx) of the plane's W1 rows / W2 rows.  [ylo, yhi): the rows that hold data (the rest of the
 // column is taken as zero without being read: the expanded grids of cm_expand.cuh); the whole column by default.
@@ -460,20 +460,6 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd(const double2 *__r
     y_fwd_body<T>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
 }
 
-// the same kernel compiled for 3 CTAs per SM (168 registers): used at N = 256
-template <int T>
-__global__ void __launch_bounds__(kThreads, 3) k_y_fwd_occ3(const double2 *__restrict__ W1, double2 *__restrict__ W2,
-                                                    const double2 *__restrict__ tw)
-{
-    constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
-    extern __shared__ double2 smem[];
-    const int tid = threadIdx.x, px = tid & 7, g = tid / (8 * T);
-    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
-    const size_t bz = q / NN;
-    const int sx = (int)(q % NN);
-    y_fwd_body<T>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
-}
-
 // P2 split by output parity: 256 threads, warps 0-3 form the even slots (P = 0), warps 4-7 the odd ones
 // (P = 1) of the SAME columns.  The two halves of a forward transform share nothing but their input, so
 // each thread carries one half only: about half the registers, twice the warps per SM (latency hiding),
@@ -508,7 +494,7 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *
 
 // ================================ P4: y inverse ====================================
 template <int T>
-__global__ void __launch_bounds__(batch_threads<T>(), T == 16 ? 3 : (T == 32 ? 1 : 2)) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
+__global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
                                                     const double2 *__restrict__ tw)
 {
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();

@@ -79,7 +79,6 @@ template <int T> int set_attrs(cm_plan *p)
     if constexpr (T <= 16) {
         CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
         CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-        CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_occ3<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
         CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_tma<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZConvCfg<T>::SMEM));
         if constexpr (T >= 8)
             CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_warp<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZWarpCfg<T>::SMEM));
@@ -153,9 +152,6 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     if constexpr (T <= 16) {
         if (p->split_y) {
             k_y_fwd_split<T><<<(unsigned)(planes * NN / PEN), 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
-            done_y = true;
-        } else if (T == 16) {
-            k_y_fwd_occ3<T><<<(unsigned)(planes * NN / PEN), kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
             done_y = true;
         }
     }
@@ -359,8 +355,8 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
     }
     if (rc == CM_OK) {
         // kernel variants by size, each chosen by measurement
-        p->split_y = (N == 256);      // P2 split by output parity: -5 % at N = 256, neutral or worse below
-        p->split_x = (N == 256);      // P1 split by output parity: -14 % at N = 256, +6 % at N = 128
+        p->split_y = (N == 256);      // P2 split by output parity: -8 % at N = 256, +4 % at N = 128
+        p->split_x = (N == 256);      // P1 split by output parity: -12 % at N = 256, +7 % at N = 128
         p->zconv_warp = (N == 128);   // warp-autonomous P3: -6 % at N = 128; at N = 256 its 32-byte TMA boxes crawl
         int dev = 0;
         if (cuda_fail(p, cudaGetDevice(&dev), "cudaGetDevice") ||

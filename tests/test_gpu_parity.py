@@ -397,3 +397,30 @@ def test_two_level_nest_at_512_whole_grid_and_host_entry_point():
     _assert_parity(got, ref)
     errs = [float(np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(L)]
     print("PARITY 2 x 512^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))
+
+
+@pytest.mark.parametrize("N,L", [(64, 3), (128, 3), (256, 2)])
+def test_results_do_not_depend_on_what_else_runs_on_the_gpu(N, L):
+    """Race witness (compute-sanitizer is closed on this pool, profiles/r02_sanitizer.md): the hand-rolled
+    mbarrier / TMA / named-barrier protocols of P3 and the programmatic dependent launches of P5 must give the same
+    bits whatever the residency and timing of their CTAs.  The solve is repeated alone and while a second stream
+    keeps the SMs busy with unrelated kernels (large matmuls and copies that evict L2 and steal CTA slots)."""
+    pkg = _pkg()
+    rng = np.random.default_rng(99 + N)
+    rho = torch.from_numpy(rng.random((L, N, N, N))).cuda()
+    plan = pkg.Plan(N, L, 2.0 / N)
+    ref = plan.potential(rho).clone()
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    a = torch.randn(4096, 4096, device="cuda")
+    big = torch.empty(64 << 20, dtype=torch.float32, device="cuda")
+    out = torch.empty_like(ref)
+    for rep in range(6):
+        with torch.cuda.stream(side):
+            for _ in range(3 + rep):
+                a = (a @ a).clamp_(-1.0, 1.0)
+                big.add_(1.0)
+        plan.potential(rho, out)
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref), f"repeat {rep}: result changed under co-scheduling"
+    plan.close()
