@@ -155,6 +155,16 @@ int cm_potential_modified(cm_plan *plan, const double *rho_levels, double *phi_l
 int cm_potential_modified_triplets(cm_plan *plan, const double *rho_levels, double *phi_levels, int qdp_direct, void *stream);
 
 /*
+ * Allocate what cm_potential_modified (depth = 2) or cm_potential_modified_triplets (depth = 3; qdp_direct as there)
+ * needs beyond the plan itself — the single-level plans of the doubled / quadrupled grids with their K-hat, and compact
+ * N^3 buffers — so that the calls themselves only enqueue (one CUDA-graph launch per call, captured on the first call per
+ * (rho, phi) pair).  Optional: the two calls do the same on first use, synchronising the device once.  Idempotent;
+ * all or nothing (CM_ENOMEM leaves the plan as it was).  CM_EINVAL for sizes the calls reject, CM_ENOTREADY before
+ * cm_green_precompute.
+ */
+int cm_plan_prepare_modified(cm_plan *plan, int depth, int qdp_direct);
+
+/*
  * Direct fine -> coarse summation (Eq. B.7): the input of grid `src_level`
  * to the potential on the coarser grid `dst_level`,
  *     Phi_ds(t) = -G sum_s rho_s dx_src^3 / |r_t - r_s|        (cell centres; all N^3 cells s of the source grid),

@@ -17,7 +17,7 @@ CM_OK, CM_EINVAL, CM_ENOMEM, CM_ECUDA, CM_ENOTREADY = 0, -1, -2, -3, -4
 CM_BUF_RESTRICTED, CM_BUF_HOLE, CM_BUF_KHAT = 0, 1, 2
 
 EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potential_host", "cm_potential_profile",
-           "cm_acceleration", "cm_potential_modified", "cm_potential_modified_triplets", "cm_direct_sum",
+           "cm_acceleration", "cm_potential_modified", "cm_potential_modified_triplets", "cm_plan_prepare_modified", "cm_direct_sum",
            "cm_plan_destroy",
            "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
            "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error"]
@@ -45,6 +45,7 @@ def lib() -> C.CDLL:
     L.cm_potential_modified.argtypes = [vp, vp, vp, vp]
     L.cm_direct_sum.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
     L.cm_potential_modified_triplets.argtypes = [vp, vp, vp, C.c_int, vp]
+    L.cm_plan_prepare_modified.argtypes = [vp, C.c_int, C.c_int]
     L.cm_plan_destroy.argtypes = [vp]
     L.cm_plan_set_G.argtypes = [vp, C.c_double]
     L.cm_plan_workspace_bytes.argtypes = [vp]
@@ -100,6 +101,10 @@ def cm_potential_modified(plan: int, rho_ptr: int, phi_ptr: int, stream: int = 0
 
 def cm_potential_modified_triplets(plan: int, rho_ptr: int, phi_ptr: int, qdp_direct: int = 0, stream: int = 0) -> None:
     _check(lib().cm_potential_modified_triplets(plan, rho_ptr, phi_ptr, int(qdp_direct), stream), plan)
+
+
+def cm_plan_prepare_modified(plan: int, depth: int, qdp_direct: int = 0) -> None:
+    _check(lib().cm_plan_prepare_modified(plan, int(depth), int(qdp_direct)), plan)
 
 
 def cm_direct_sum(plan: int, rho_ptr: int, src_level: int, dst_level: int, phi_ptr: int, stream: int = 0) -> None:
@@ -186,6 +191,10 @@ class Plan:
         s = torch.cuda.current_stream(rho.device).cuda_stream if stream is None else int(stream)
         cm_potential_modified_triplets(self._h, rho.data_ptr(), phi.data_ptr(), int(bool(qdp_direct)), s)
         return phi
+
+    def prepare_modified(self, depth: int = 2, qdp_direct: bool = False):
+        """Allocate the expanded-grid plans of the modified method up front (cm_plan_prepare_modified)."""
+        cm_plan_prepare_modified(self._h, depth, int(bool(qdp_direct)))
 
     def direct_sum(self, rho, src_level: int, dst_level: int, stream=None):
         """Eq. B.7: potential of level src_level's mass on the cells of level dst_level, [N, N, N]."""

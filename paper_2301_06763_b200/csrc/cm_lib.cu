@@ -18,6 +18,7 @@ namespace {
 struct GraphEntry {
     const double *rho;
     double *phi;
+    int mode;                      // 0 cm_potential, 1 pairs, 2 triplets (quadrupled grid by FFT), 3 triplets (Eq. B.7)
     cudaGraphExec_t exec;
     unsigned long long last_use;   // for least-recently-used eviction
 };
@@ -34,7 +35,6 @@ struct cm_plan {
     size_t bytes = 0;
     bool green_ready = false;
     bool split_x = false, split_y = false;   // P1 / P2 split by output parity (256-thread CTAs): N = 256
-    int hole_all = 0;               // P5 keeps Phi_hole + ext on every cell (cm_potential_modified)
     cm_plan *dbl = nullptr, *qdp = nullptr;   // single-level plans of the doubled (2N)^3 and quadrupled (4N)^3 fine grid
     double *rho4 = nullptr, *phi4 = nullptr, *tmp3 = nullptr;
     double *rho2 = nullptr, *phi2 = nullptr;   // two doubled grids each: one complex solve serves two pairs
@@ -114,7 +114,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
 // that this level's loads and transforms overlap that level's tail; the kernel waits (griddepcontrol.wait) only
 // before it reads what level b-1 wrote.
 template <int T>
-void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid, double scale0, bool chained)
+void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid, double scale0, bool chained, int hole_all)
 {
     constexpr int N = 16 * T;
     cudaLaunchConfig_t cfg = {};
@@ -128,13 +128,13 @@ void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid,
     cfg.attrs = at;
     cfg.numAttrs = chained ? 1 : 0;
     cudaLaunchKernelEx(&cfg, k_x_inv<T>, (const double2 *)p->W1, phi, p->hole, (const double *)p->hole, (const double2 *)p->tw, p->L,
-                       scale0, (size_t)b * N * N, p->hole_all);
+                       scale0, (size_t)b * N * N, hole_all);
 }
 
 // The five FFT passes (steps a3-a7) with the prolongation + Eq. 14 sum (a8) folded into P5:
 // P1-P4 take every level in one launch; P5 runs level by level, coarse -> fine, because
 // level b adds the prolonged hole potentials of level b-1 (k_x_inv).
-template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev)
+template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev, int hole_all)
 {
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
     const int L = p->L;
@@ -163,7 +163,7 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     if (ev) cudaEventRecord(ev[5], s);
     const size_t lrows = (size_t)N * N;
     const unsigned gl = (unsigned)((lrows + ROWS - 1) / ROWS);
-    for (int b = 0; b < L; ++b) launch_x_inv<T>(p, phi, s, b, gl, scale0, /*chained=*/b > 0);
+    for (int b = 0; b < L; ++b) launch_x_inv<T>(p, phi, s, b, gl, scale0, /*chained=*/b > 0, hole_all);
     if (ev) cudaEventRecord(ev[6], s);
     p->launches += 4 + L;
     CM_CUDA(p, cudaGetLastError());
@@ -187,7 +187,7 @@ template <int T> void level_p5(cm_plan *p, double *phi, cudaStream_t s, int l)
 {
     constexpr int N = 16 * T, ROWS = kThreads / T;
     const size_t lrows = (size_t)N * N;
-    launch_x_inv<T>(p, phi, s, l, (unsigned)((lrows + ROWS - 1) / ROWS), -p->G * p->dx0 * p->dx0, /*chained=*/false);
+    launch_x_inv<T>(p, phi, s, l, (unsigned)((lrows + ROWS - 1) / ROWS), -p->G * p->dx0 * p->dx0, /*chained=*/false, 0);
 }
 void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int l, bool p5)
 {
@@ -202,7 +202,8 @@ void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, 
 }
 
 // ev (optional): 8 events; ev[0] start, ev[1] after a1, ev[2..6] after P1..P5, ev[7] after a8
-int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev = nullptr)
+// hole_all: P5 keeps H = Phi_hole + ext on every cell, not only on the ring the next level reads (the modified method, Eq. B.1)
+int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev = nullptr, int hole_all = 0)
 {
     const int N = p->N, L = p->L, H = N / 2;
     const size_t n3 = (size_t)N * N * N, h3 = (size_t)H * H * H;
@@ -218,12 +219,12 @@ int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cu
     if (ev) cudaEventRecord(ev[1], s);
     int rcode = CM_EINVAL;
     switch (p->T) {
-        case 1: rcode = launch_passes<1>(p, rho, phi, s, ev); break;
-        case 2: rcode = launch_passes<2>(p, rho, phi, s, ev); break;
-        case 4: rcode = launch_passes<4>(p, rho, phi, s, ev); break;
-        case 8: rcode = launch_passes<8>(p, rho, phi, s, ev); break;
-        case 16: rcode = launch_passes<16>(p, rho, phi, s, ev); break;
-        case 32: rcode = launch_passes<32>(p, rho, phi, s, ev); break;
+        case 1: rcode = launch_passes<1>(p, rho, phi, s, ev, hole_all); break;
+        case 2: rcode = launch_passes<2>(p, rho, phi, s, ev, hole_all); break;
+        case 4: rcode = launch_passes<4>(p, rho, phi, s, ev, hole_all); break;
+        case 8: rcode = launch_passes<8>(p, rho, phi, s, ev, hole_all); break;
+        case 16: rcode = launch_passes<16>(p, rho, phi, s, ev, hole_all); break;
+        case 32: rcode = launch_passes<32>(p, rho, phi, s, ev, hole_all); break;
     }
     if (rcode != CM_OK) return rcode;
     // a8 (prolongation + Eq. 14 sum) ran inside P5
@@ -296,6 +297,47 @@ int make_tensor_maps(cm_plan *p)
             return CM_ECUDA;
         }
     }
+    return CM_OK;
+}
+
+// One call = one CUDA-graph launch.  The sequence of `mode` (0: the original method; 1-3: the modified method, whose
+// expanded-grid plans must already exist — nothing may allocate during capture) is captured once per (rho, phi, mode) on the
+// plan's own stream and launched on the caller's; the cache keeps the kGraphCacheSize most recently used entries (callers
+// that rotate buffers should reuse them).  CM_DEBUG=nograph launches kernel by kernel.
+int enqueue_mode(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int mode);
+
+int run_graphed(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int mode)
+{
+    if (!p->use_graph) return enqueue_mode(p, rho, phi, s, mode);
+    for (auto &g : p->graphs)
+        if (g.rho == rho && g.phi == phi && g.mode == mode) {
+            g.last_use = ++p->use_counter;
+            CM_CUDA(p, cudaGraphLaunch(g.exec, s));
+            return CM_OK;
+        }
+    cudaGraph_t graph = nullptr;
+    CM_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
+    const int rc = enqueue_mode(p, rho, phi, p->cap_stream, mode);
+    cudaError_t ee = cudaStreamEndCapture(p->cap_stream, &graph);
+    if (rc != CM_OK || ee != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        if (rc != CM_OK) return rc;
+        CM_CUDA(p, ee);
+    }
+    GraphEntry ge{rho, phi, mode, nullptr, ++p->use_counter};
+    ee = cudaGraphInstantiate(&ge.exec, graph, 0);
+    cudaGraphDestroy(graph);   // the executable graph is self-contained
+    CM_CUDA(p, ee);
+    if (p->graphs.size() >= kGraphCacheSize) {
+        size_t lru = 0;
+        for (size_t i = 1; i < p->graphs.size(); ++i)
+            if (p->graphs[i].last_use < p->graphs[lru].last_use) lru = i;
+        cudaGraphExecDestroy(p->graphs[lru].exec);
+        p->graphs[lru] = ge;
+    } else {
+        p->graphs.push_back(ge);
+    }
+    CM_CUDA(p, cudaGraphLaunch(ge.exec, s));
     return CM_OK;
 }
 
@@ -421,41 +463,7 @@ int cm_potential(cm_plan *p, const double *rho, double *phi, void *stream)
     if (!p->green_ready) return CM_ENOTREADY;
     const size_t tot = (size_t)p->L * p->N * p->N * p->N;
     if ((rho <= phi && phi < rho + tot) || (phi <= rho && rho < phi + tot)) return CM_EINVAL;
-    cudaStream_t s = (cudaStream_t)stream;
-    if (!p->use_graph) return enqueue_solve(p, rho, phi, s);
-
-    for (auto &g : p->graphs)
-        if (g.rho == rho && g.phi == phi) {
-            g.last_use = ++p->use_counter;
-            CM_CUDA(p, cudaGraphLaunch(g.exec, s));
-            return CM_OK;
-        }
-    // capture once per (rho, phi) pair on the plan's own stream, launch on the caller's; the cache keeps the
-    // kGraphCacheSize most recently used pairs (callers that rotate buffers should reuse them)
-    cudaGraph_t graph = nullptr;
-    CM_CUDA(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
-    const int rc = enqueue_solve(p, rho, phi, p->cap_stream);
-    cudaError_t ee = cudaStreamEndCapture(p->cap_stream, &graph);
-    if (rc != CM_OK || ee != cudaSuccess) {
-        if (graph) cudaGraphDestroy(graph);
-        if (rc != CM_OK) return rc;
-        CM_CUDA(p, ee);
-    }
-    GraphEntry ge{rho, phi, nullptr, ++p->use_counter};
-    ee = cudaGraphInstantiate(&ge.exec, graph, 0);
-    cudaGraphDestroy(graph);   // the executable graph is self-contained
-    CM_CUDA(p, ee);
-    if (p->graphs.size() >= kGraphCacheSize) {
-        size_t lru = 0;
-        for (size_t i = 1; i < p->graphs.size(); ++i)
-            if (p->graphs[i].last_use < p->graphs[lru].last_use) lru = i;
-        cudaGraphExecDestroy(p->graphs[lru].exec);
-        p->graphs[lru] = ge;
-    } else {
-        p->graphs.push_back(ge);
-    }
-    CM_CUDA(p, cudaGraphLaunch(ge.exec, s));
-    return CM_OK;
+    return run_graphed(p, rho, phi, (cudaStream_t)stream, 0);
 }
 
 int cm_potential_profile(cm_plan *p, const double *rho, double *phi, void *stream, float *ms_host, int n_ms)
@@ -544,7 +552,7 @@ namespace {
 // forward passes pruned to the central Nc^3 block, inverse passes decimated by F.  src_re / src_im: compact Nc^3
 // densities (src_im optional: the second real field); out_re / out_im: minus the block SUMS of their potentials.
 template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, const double *src_im, double *out_re, double *out_im,
-                                            cudaStream_t s)
+                                            cudaStream_t s, bool attrs_only)
 {
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>(), Nc = N / F,
                   c0 = (N - Nc) / 2;
@@ -557,6 +565,7 @@ template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, c
         CM_CUDA(pe, cudaFuncSetAttribute(k_x_inv_dec<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
         attrs = true;
     }
+    if (attrs_only) return CM_OK;
     k_x_fwd_blk<T><<<(unsigned)(Nc * Nc / ROWS), kThreads, smem_row<T>(), s>>>(src_re, src_im, pe->W1, pe->tw, Nc, c0);
     k_y_fwd_blk<T><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W1, pe->W2, pe->tw, Nc, c0);
     k_z_conv_dec<T, F><<<(unsigned)((size_t)(N + 1) * (NN / PEN)), BT, ZDecCfg<T>::SMEM, s>>>(pe->Khat, pe->W2, pe->tw, pe->decE, c0, c0 + Nc);
@@ -566,10 +575,11 @@ template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, c
     return CM_OK;
 }
 
-int dispatch_expanded(cm_plan *pe, int F, const double *src_re, const double *src_im, double *out_re, double *out_im, cudaStream_t s)
+int dispatch_expanded(cm_plan *pe, int F, const double *src_re, const double *src_im, double *out_re, double *out_im, cudaStream_t s,
+                      bool attrs_only = false)
 {
 #define CM_EXP(TT, FF) \
-    if (pe->T == TT && F == FF) return expanded_passes<TT, FF>(pe, src_re, src_im, out_re, out_im, s);
+    if (pe->T == TT && F == FF) return expanded_passes<TT, FF>(pe, src_re, src_im, out_re, out_im, s, attrs_only);
     CM_EXP(2, 2) CM_EXP(4, 2) CM_EXP(8, 2) CM_EXP(16, 2) CM_EXP(32, 2)
     CM_EXP(4, 4) CM_EXP(8, 4) CM_EXP(16, 4) CM_EXP(32, 4)
 #undef CM_EXP
@@ -606,6 +616,7 @@ int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **src, double **re
             if (cuda_fail(p, cudaMemcpy(pe->decE, E.data(), n * sizeof(double2), cudaMemcpyHostToDevice), "cudaMemcpy(E)")) rc = CM_ECUDA;
         }
     }
+    if (rc == CM_OK) rc = dispatch_expanded(*plan, F, nullptr, nullptr, nullptr, nullptr, nullptr, /*attrs_only=*/true);
     if (rc == CM_OK && !*src) rc = dev_alloc(p, src, 2 * n3);
     if (rc == CM_OK && !*res) rc = dev_alloc(p, res, 2 * n3);
     if (rc != CM_OK) {
@@ -639,20 +650,27 @@ int solve_expanded(cm_plan *p, cm_plan *pe, int F, const double *rho, double *sr
 int direct_sum_impl(cm_plan *p, const double *rho_src, int src_level, int dst_level, double *phi_dst, cudaStream_t s);
 
 // depth 2: Eq. B.1-B.2 (pairs); depth 3: Eq. B.3-B.6 (triplets), the quadrupled grid by FFT or by Eq. B.7
+// everything the modified method allocates (expanded-grid plans with their K-hat, compact buffers): idempotent, all or
+// nothing; runs before any capture
+int modified_prepare(cm_plan *p, int depth, int qdp_direct)
+{
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    int rc = CM_OK;
+    if (p->L > 1 && (rc = ensure_expanded(p, 2, &p->dbl, &p->rho2, &p->phi2)) != CM_OK) return rc;
+    const bool triple = depth == 3 && p->L > 2;
+    if (triple && !qdp_direct && (rc = ensure_expanded(p, 4, &p->qdp, &p->rho4, &p->phi4)) != CM_OK) return rc;
+    if (triple && qdp_direct && !p->tmp3 && (rc = dev_alloc(p, &p->tmp3, 2 * n3)) != CM_OK) return rc;
+    return CM_OK;
+}
+
 int modified_impl(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int depth, int qdp_direct)
 {
     const int N = p->N, L = p->L;
     const size_t n3 = (size_t)N * N * N;
     const unsigned gn = (unsigned)((n3 + 255) / 256);
-    int rc = CM_OK;
-    if (L > 1 && (rc = ensure_expanded(p, 2, &p->dbl, &p->rho2, &p->phi2)) != CM_OK) return rc;
     const bool triple = depth == 3 && L > 2;
-    if (triple && !qdp_direct && (rc = ensure_expanded(p, 4, &p->qdp, &p->rho4, &p->phi4)) != CM_OK) return rc;
-    if (triple && qdp_direct && !p->tmp3 && (rc = dev_alloc(p, &p->tmp3, 2 * n3)) != CM_OK) return rc;
     // the original solve, keeping H_n = Phi_hole^n + ext_n on every cell; the finest level's Phi is final (B.2 / B.6)
-    p->hole_all = 1;
-    rc = enqueue_solve(p, rho, phi, s);
-    p->hole_all = 0;
+    int rc = enqueue_solve(p, rho, phi, s, nullptr, /*hole_all=*/1);
     if (rc != CM_OK) return rc;
     // doubled grids: Phi(Omega^n) = H_n + reduce(Phi_dbl^{n+1}), two pairs per complex solve; in the triplet scheme the
     // doubled grid has a central hole (grid n+2's mass comes through the quadrupled grid) except for the last pair (B.5)
@@ -689,6 +707,17 @@ int modified_impl(cm_plan *p, const double *rho, double *phi, cudaStream_t s, in
     return CM_OK;
 }
 
+int enqueue_mode(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int mode)
+{
+    switch (mode) {
+        case 0: return enqueue_solve(p, rho, phi, s);
+        case 1: return modified_impl(p, rho, phi, s, 2, 0);
+        case 2: return modified_impl(p, rho, phi, s, 3, 0);
+        case 3: return modified_impl(p, rho, phi, s, 3, 1);
+    }
+    return CM_EINVAL;
+}
+
 int check_modified_args(cm_plan *p, const double *rho, double *phi)
 {
     if (!p || !rho || !phi) return CM_EINVAL;
@@ -708,7 +737,9 @@ int cm_potential_modified(cm_plan *p, const double *rho, double *phi, void *stre
     const int rc = check_modified_args(p, rho, phi);
     if (rc != CM_OK) return rc;
     if (p->N > 256) return CM_EINVAL;                      // the doubled grid must be a supported size (2N <= 512)
-    return modified_impl(p, rho, phi, (cudaStream_t)stream, 2, 0);
+    const int rp = modified_prepare(p, 2, 0);
+    if (rp != CM_OK) return rp;
+    return run_graphed(p, rho, phi, (cudaStream_t)stream, 1);
 }
 
 int cm_potential_modified_triplets(cm_plan *p, const double *rho, double *phi, int qdp_direct, void *stream)
@@ -716,7 +747,17 @@ int cm_potential_modified_triplets(cm_plan *p, const double *rho, double *phi, i
     const int rc = check_modified_args(p, rho, phi);
     if (rc != CM_OK) return rc;
     if (p->N > 256 || (!qdp_direct && p->N > 128)) return CM_EINVAL;   // 2N (and 4N) must be supported sizes (<= 512)
-    return modified_impl(p, rho, phi, (cudaStream_t)stream, 3, qdp_direct ? 1 : 0);
+    const int rp = modified_prepare(p, 3, qdp_direct ? 1 : 0);
+    if (rp != CM_OK) return rp;
+    return run_graphed(p, rho, phi, (cudaStream_t)stream, qdp_direct ? 3 : 2);
+}
+
+int cm_plan_prepare_modified(cm_plan *p, int depth, int qdp_direct)
+{
+    if (!p || (depth != 2 && depth != 3)) return CM_EINVAL;
+    if (!p->green_ready) return CM_ENOTREADY;
+    if (p->N > 256 || (depth == 3 && !qdp_direct && p->N > 128)) return CM_EINVAL;
+    return modified_prepare(p, depth, qdp_direct ? 1 : 0);
 }
 
 int cm_direct_sum(cm_plan *p, const double *rho_levels, int src_level, int dst_level, double *phi_dst, void *stream)

@@ -151,6 +151,37 @@ def test_triplets_random_levels(N, L, direct):
     _assert_parity(pairs, oracle.solve_modified(rho, 2.0 / N, G=1.7))
 
 
+def test_prepare_call_and_graph_replay_give_the_same_bits():
+    """cm_plan_prepare_modified allocates the expanded-grid plans up front; the calls are then one CUDA-graph launch each
+    (captured per (rho, phi, scheme)); CM_DEBUG=nograph launches the same kernels one by one."""
+    import os
+    import paper_2301_06763_b200 as pkg
+    rng = np.random.default_rng(5)
+    rho = torch.from_numpy(rng.random((4, 32, 32, 32))).cuda()
+    plan = pkg.Plan(32, 4, 0.05)
+    before = plan.workspace_bytes
+    plan.prepare_modified(3)
+    assert plan.workspace_bytes > before
+    grown = plan.workspace_bytes
+    a = plan.potential_modified_triplets(rho)
+    b = plan.potential_modified(rho)
+    a2 = plan.potential_modified_triplets(rho, a.clone().zero_())
+    o = plan.potential(rho)
+    torch.cuda.synchronize()
+    assert plan.workspace_bytes == grown and torch.equal(a, a2) and not torch.equal(a, b) and not torch.equal(b, o)
+    plan.close()
+    os.environ["CM_DEBUG"] = "nograph"
+    try:
+        plan2 = pkg.Plan(32, 4, 0.05)
+        a3 = plan2.potential_modified_triplets(rho)
+        b3 = plan2.potential_modified(rho)
+        torch.cuda.synchronize()
+        assert torch.equal(a3, a) and torch.equal(b3, b)
+        plan2.close()
+    finally:
+        del os.environ["CM_DEBUG"]
+
+
 def test_triplets_dipole_two_levels_down():
     N, L, dx0 = 16, 3, 0.125
     rho = np.zeros((L, N, N, N))
