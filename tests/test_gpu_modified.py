@@ -221,3 +221,31 @@ def test_triplets_n128_every_cell_against_the_oracle():
     _assert_parity(got, ref)
     errs = [float(np.abs(got[l] - ref[l]).max() / np.abs(ref[l]).max()) for l in range(L)]
     print(f"PARITY cm_potential_modified_triplets {L} x 128^3, whole grid: " + " ".join(f"{e:.2e}" for e in errs))
+
+
+def test_out_of_memory_while_building_the_expanded_plan_is_clean_and_recoverable():
+    """a failure half-way through the lazy set-up of the doubled-grid plan must leave nothing behind.  Device
+    memory is filled so that the plan of the doubled grid fits but the scratch of its K-hat does not: the call returns
+    CM_ENOMEM, the workspace figure is unchanged, and once memory is back the same call works and matches the oracle."""
+    import paper_2301_06763_b200 as pkg
+    N, L, dx0 = 64, 2, 2.0 / 64
+    rng = np.random.default_rng(64)
+    rho_h = rng.random((L, N, N, N))
+    rho = torch.from_numpy(rho_h).cuda()
+    plan = pkg.Plan(N, L, dx0)
+    before = plan.workspace_bytes
+    torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    hog = torch.empty(free - (450 << 20), dtype=torch.uint8, device="cuda")     # leave ~450 MB
+    with pytest.raises(pkg.CMError) as ei:
+        plan.potential_modified(rho)
+    assert ei.value.code == pkg.CM_ENOMEM, ei.value
+    assert plan.workspace_bytes == before
+    with pytest.raises(pkg.CMError):                      # still a clean error, not a half-built plan
+        plan.potential_modified(rho)
+    del hog
+    torch.cuda.empty_cache()
+    got = plan.potential_modified(rho).cpu().numpy()
+    _assert_parity(got, oracle.solve_modified(rho_h, dx0))
+    plan.close()
