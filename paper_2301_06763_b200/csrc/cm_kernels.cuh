@@ -105,6 +105,9 @@ template <int P, class Tw> __device__ __forceinline__ double2 tw_next(const Tw &
 }
 
 // ---- half transforms ---------------------------------------------------------------
+// element (row, col) of a pencil's exchange matrix
+template <class Lay> __device__ __forceinline__ double2 &ex_at(double2 *sm, int row, int col) { return sm[row * Lay::RS + col]; }
+
 // Forward, parity P: a[r] = input element n = j + T r (r < 16).  On return
 // v[cc*T + k2] is the spectrum value of slot  P*N + 16*k2 + cc*T + j.
 // PRE: synchronise before writing the exchange buffer (needed when one buffer serves
@@ -124,14 +127,14 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
         for (int k1 = 0; k1 < 16; ++k1) {
             const double2 t = tw_next<P>(tw, k1, twc);
             if (k1 > 0 || P) b[k1] = cmul(b[k1], t);
-            sm[k1 * Lay::RS + j] = b[k1];
+            ex_at<Lay>(sm, k1, j) = b[k1];
         }
         sync();
         if constexpr (T <= 16) {
 #pragma unroll
             for (int cc = 0; cc < 16 / T; ++cc) {
 #pragma unroll
-                for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = sm[(cc * T + j) * Lay::RS + jj];
+                for (int jj = 0; jj < T; ++jj) v[cc * T + jj] = ex_at<Lay>(sm, cc * T + j, jj);
                 Dft<T, -1>::run(&v[cc * T]);
             }
         } else {
@@ -141,7 +144,7 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
             const int q = j >> 4, c = j & 15;
             const double sg = q ? -1.0 : 1.0;
 #pragma unroll
-            for (int jj = 0; jj < 16; ++jj) v[jj] = cmfft::cfma(sg, sm[c * Lay::RS + jj + 16], sm[c * Lay::RS + jj]);
+            for (int jj = 0; jj < 16; ++jj) v[jj] = cmfft::cfma(sg, ex_at<Lay>(sm, c, jj + 16), ex_at<Lay>(sm, c, jj));
             if (q) cmfft::Dft16Mod<-1>::run(v);
             else Dft<16, -1>::run(v);
         }
@@ -177,7 +180,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
                     Dft<T, +1>::run(&v[cc * T]);
                 }
 #pragma unroll
-                for (int jj = 0; jj < T; ++jj) sm[(cc * T + j) * Lay::RS + jj] = v[cc * T + jj];
+                for (int jj = 0; jj < T; ++jj) ex_at<Lay>(sm, cc * T + j, jj) = v[cc * T + jj];
             }
             sync();
         } else {
@@ -210,15 +213,15 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
                 for (int m = 0; m < 16; ++m) y[m] = v[m];
             }
 #pragma unroll
-            for (int jj = 0; jj < 16; ++jj) sm[c * Lay::RS + 16 * q + jj] = y[jj];
+            for (int jj = 0; jj < 16; ++jj) ex_at<Lay>(sm, c, 16 * q + jj) = y[jj];
             sync();
         }
         if (DEC > 1 && (j % DEC) != 0) return;
         TwCarry twc{make_double2(1.0, 0.0), make_double2(1.0, 0.0)};
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
-            if constexpr (T <= 16) w[k1] = sm[k1 * Lay::RS + j];
-            else w[k1] = cmfft::cfma((j >> 4) ? -1.0 : 1.0, sm[k1 * Lay::RS + 16 + (j & 15)], sm[k1 * Lay::RS + (j & 15)]);
+            if constexpr (T <= 16) w[k1] = ex_at<Lay>(sm, k1, j);
+            else w[k1] = cmfft::cfma((j >> 4) ? -1.0 : 1.0, ex_at<Lay>(sm, k1, 16 + (j & 15)), ex_at<Lay>(sm, k1, j & 15));
             const double2 t = tw_next<P>(tw, k1, twc);
             if (k1 > 0 || P) w[k1] = cmulc(w[k1], t);
         }

@@ -40,6 +40,10 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
     asm volatile(
@@ -248,10 +252,6 @@ template <int T> struct ZWarpCfg {
 // three __syncthreads of a tile, 5 % at the TMA waits behind them), and the four warps drift apart, so that one
 // warp's exchanges fall under another warp's butterflies.  Only the K-hat tile is shared: a warp reports when it
 // is through with a group's tile (bar_kfree, 4 arrivals), warp 0 then fetches the next one.
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
-}
 
 template <int T>
 __global__ void __launch_bounds__(kThreads, 2)
