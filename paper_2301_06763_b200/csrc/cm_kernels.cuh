@@ -757,41 +757,30 @@ __global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, 
     }
 }
 
-// ============ f-2: modified ("dipole") method, Eq. 15 / B.1-B.2 (pairs) and B.3-B.6 (triplets) ============
-// out = the fine grid l1 expanded F times (Fig. 14: F = 2, the doubled grid; L448 Fig. B.1: F = 4, the
-// quadrupled grid; F = 1: the grid itself): (F N)^3 cells of the fine size, concentric; the fine grid's density
-// (finer levels projected onto it: rc) in the central N^3, zero around; `hole`: its own cavity zeroed as well
-// (the doubled grid "with a central hole" of the triplet scheme, so that grid l1+1's mass is not counted twice).
-__global__ void k_pad_expand(int N, int F, int hole, int l1, int L, const double *__restrict__ rho, const double *__restrict__ rc,
-                             double *__restrict__ out)
+// ========================= f-2: modified method, Eq. 15 / B.1-B.6 — sources and sums ==========================
+// rho-bar of level l1 as a compact N^3 array: the level's density with the finer levels projected onto it (rc);
+// `hole`: its own cavity zeroed (the doubled grid "with a central hole" of the triplet scheme, so that grid l1+1's
+// mass is not counted twice).  The expanded grid around it is never materialised (cm_expand.cuh).
+__global__ void k_level_density(int N, int hole, int l1, int L, const double *__restrict__ rho, const double *__restrict__ rc,
+                                double *__restrict__ out)
 {
-    const int n = F * N, h = (F - 1) * N / 2, H = N / 2, Q = N / 4;
-    const size_t tot = (size_t)n * n * n, n3 = (size_t)N * N * N;
+    const int H = N / 2, Q = N / 4;
+    const size_t n3 = (size_t)N * N * N;
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= tot) return;
-    const int i = (int)(idx % n) - h, j = (int)((idx / n) % n) - h, k = (int)(idx / ((size_t)n * n)) - h;
+    if (idx >= n3) return;
+    const int i = (int)(idx % N), j = (int)((idx / N) % N), k = (int)(idx / ((size_t)N * N));
+    const bool cav = in_cavity1(k, N) && in_cavity1(j, N) && in_cavity1(i, N);
     double v = 0.0;
-    if (i >= 0 && i < N && j >= 0 && j < N && k >= 0 && k < N) {
-        const bool cav = in_cavity1(k, N) && in_cavity1(j, N) && in_cavity1(i, N);
-        if (!(cav && hole))
-            v = (cav && l1 < L - 1) ? rc[(size_t)l1 * (n3 / 8) + ((size_t)(k - Q) * H + (j - Q)) * H + (i - Q)]
-                                    : rho[(size_t)l1 * n3 + ((size_t)k * N + j) * N + i];
-    }
+    if (!(cav && hole))
+        v = (cav && l1 < L - 1) ? rc[(size_t)l1 * (n3 / 8) + ((size_t)(k - Q) * H + (j - Q)) * H + (i - Q)] : rho[(size_t)l1 * n3 + idx];
     out[idx] = v;
 }
 
-// phi_n = base + scale * (mean of the F^3 cells of `big` ((F N)^3) under each cell)   (the "reduce" of B.1 / B.3)
-__global__ void k_add_block_mean(int N, int F, const double *base, const double *__restrict__ big, double scale, double *phi_n)
+// phi_n = base + scale * add   (the "reduce" of B.1 / B.3: `add` holds the block sums the decimated passes formed)
+__global__ void k_add_scaled(size_t n, const double *base, const double *__restrict__ add, double scale, double *phi_n)
 {
-    const int n = F * N;
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= (size_t)N * N * N) return;
-    const int i = (int)(idx % N), j = (int)((idx / N) % N), k = (int)(idx / ((size_t)N * N));
-    double s = 0.0;
-    for (int c = 0; c < F; ++c)
-        for (int b = 0; b < F; ++b)
-            for (int a = 0; a < F; ++a) s += big[((size_t)(F * k + c) * n + (F * j + b)) * n + F * i + a];
-    phi_n[idx] = base[idx] + scale * (s / (double)(F * F * F));
+    if (idx < n) phi_n[idx] = base[idx] + scale * add[idx];
 }
 
 // ================= f-3: direct fine -> coarse summation, Eq. B.7 =================

@@ -642,8 +642,8 @@ int solve_expanded(cm_plan *p, cm_plan *pe, int F, const double *rho, double *sr
 {
     const size_t n3 = (size_t)p->N * p->N * p->N;
     const unsigned g = (unsigned)((n3 + 255) / 256);
-    k_pad_expand<<<g, 256, 0, s>>>(p->N, 1, hole1, l1, p->L, rho, p->rc, src);          // rho-bar of grid l1 (optionally holed)
-    if (l1b >= 0) k_pad_expand<<<g, 256, 0, s>>>(p->N, 1, hole1b, l1b, p->L, rho, p->rc, src + n3);
+    k_level_density<<<g, 256, 0, s>>>(p->N, hole1, l1, p->L, rho, p->rc, src);          // rho-bar of grid l1 (optionally holed)
+    if (l1b >= 0) k_level_density<<<g, 256, 0, s>>>(p->N, hole1b, l1b, p->L, rho, p->rc, src + n3);
     return dispatch_expanded(pe, F, src, l1b >= 0 ? src + n3 : nullptr, res, l1b >= 0 ? res + n3 : nullptr, s);
 }
 
@@ -681,24 +681,24 @@ int modified_impl(cm_plan *p, const double *rho, double *phi, cudaStream_t s, in
         if (rc != CM_OK) return rc;
         for (int q = 0; q < (two ? 2 : 1); ++q) {
             const double dxf = p->dx0 * std::exp2(-(double)(n + q + 1));
-            k_add_block_mean<<<gn, 256, 0, s>>>(N, 1, p->hole + (n + q) * n3, p->phi2 + q * n3, p->G * dxf * dxf / 8.0, phi + (n + q) * n3);
+            k_add_scaled<<<gn, 256, 0, s>>>(n3, p->hole + (n + q) * n3, p->phi2 + q * n3, p->G * dxf * dxf / 8.0, phi + (n + q) * n3);
         }
     }
     // quadrupled grids (B.3): + reduce(Phi_qdp^{n+2}) for n < L-2, by the same convolution or by direct summation (B.7)
     if (triple) {
         for (int n = 0; n + 2 < L; n += (qdp_direct ? 1 : 2)) {
             if (qdp_direct) {
-                k_pad_expand<<<gn, 256, 0, s>>>(N, 1, 0, n + 2, L, rho, p->rc, p->tmp3);           // rho-bar of grid n+2
+                k_level_density<<<gn, 256, 0, s>>>(N, 0, n + 2, L, rho, p->rc, p->tmp3);           // rho-bar of grid n+2
                 rc = direct_sum_impl(p, p->tmp3, n + 2, n, p->tmp3 + n3, s);
                 if (rc != CM_OK) return rc;
-                k_add_block_mean<<<gn, 256, 0, s>>>(N, 1, phi + n * n3, p->tmp3 + n3, 1.0, phi + n * n3);
+                k_add_scaled<<<gn, 256, 0, s>>>(n3, phi + n * n3, p->tmp3 + n3, 1.0, phi + n * n3);
             } else {
                 const bool two = n + 3 < L;
                 rc = solve_expanded(p, p->qdp, 4, rho, p->rho4, p->phi4, s, n + 2, 0, two ? n + 3 : -1, 0);
                 if (rc != CM_OK) return rc;
                 for (int q = 0; q < (two ? 2 : 1); ++q) {
                     const double dxf = p->dx0 * std::exp2(-(double)(n + q + 2));
-                    k_add_block_mean<<<gn, 256, 0, s>>>(N, 1, phi + (n + q) * n3, p->phi4 + q * n3, p->G * dxf * dxf / 64.0, phi + (n + q) * n3);
+                    k_add_scaled<<<gn, 256, 0, s>>>(n3, phi + (n + q) * n3, p->phi4 + q * n3, p->G * dxf * dxf / 64.0, phi + (n + q) * n3);
                 }
             }
         }

@@ -5,7 +5,7 @@
 // K-hat and the inverse z transform of one pencil happen in registers without the
 // (2N)^3 spectrum ever reaching memory.
 //
-// Why this shape (profiles/r01a_ncu_full_config5.md): the first k_z_conv was neither
+// Why this shape (round 1's first capture): the first k_z_conv was neither
 // DRAM- nor fp64-bound; its 8 warps/SM stalled on the tile load, on K-hat loads issued in
 // the middle of the dependency chain and on CTA-wide barriers.  Here
 //   (the launch covers levels b0 .. b0 + L - 1: all of them in cm_potential, one in cm_potential_host's pipeline)
@@ -19,7 +19,7 @@
 //     radix-T exchange needs __syncwarp only; twiddles come from a shared-memory copy.
 // Output is staged in shared memory (the idle exchange buffer) and written by a TMA store:
 // writing it straight from registers (32-byte sectors per row per warp with this thread
-// mapping) cost 6 ms of the 10.6 ms at N = 256 (ablation, DESIGN.md §7).
+// mapping) cost 6 ms of the 10.6 ms at N = 256 (ablation, DESIGN.md §6).
 #pragma once
 
 #include <cuda.h>
