@@ -32,10 +32,10 @@ namespace cmk {
 template <int T, int DEC> __device__ __forceinline__ int dec_j(int u) { return (u % (T / DEC)) * DEC + u / (T / DEC); }
 
 // v[i] *= E[slot of v[i]]  (E in slot order, one parity block)
-template <int T> __device__ __forceinline__ void mul_E(double2 (&v)[16], const double2 *__restrict__ Ep, int j)
+template <int T> __device__ __forceinline__ void mul_E(double2 (&v)[16], const double2 *Ep, int j)
 {
 #pragma unroll
-    for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], __ldg(Ep + vslot<T>(i, j)));
+    for (int i = 0; i < 16; ++i) v[i] = cmul(v[i], Ep[vslot<T>(i, j)]);
 }
 
 // P1 on the block: compact row rc = zc Nc + yc of the Nc^3 source sits at row (c0 + zc, c0 + yc) of the big grid, its
@@ -97,9 +97,27 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd_blk(const double2 
 template <int T> struct ZDecCfg {
     static constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     static constexpr int RSK = khat_row_stride(N);   // doubles per pencil of K-hat in global memory
-    static constexpr int RSKS = NN + 2;              // ... in shared memory: 8 pencils x 2 j of a half-warp hit 16 distinct 8-byte words
-    static constexpr uint32_t EX_BYTES = 2 * PEN * LayBatch<T>::PS * 16, KH_BYTES = PEN * RSKS * 8;
-    static constexpr uint32_t OFF_KH = EX_BYTES, OFF_BAR = OFF_KH + KH_BYTES, SMEM = OFF_BAR + 16;
+    // K-hat is even in the z frequency; in slot order the mirror of slot m of the even block is slot N - m and of the odd
+    // block N - 1 - m, so the first N/2 + 1 (even) and N/2 (odd) slots of a pencil are all of it.  Row stride N + 2: the
+    // 8 pencils x 2 j of a half-warp hit 16 distinct 8-byte words.
+    static constexpr int KE = N / 2 + 2, RSKH = N + 2;
+    static constexpr uint32_t EX_BYTES = 2 * PEN * LayBatch<T>::PS * 16, KH_BYTES = PEN * RSKH * 8, TW_BYTES = 32 * T * 16,
+                              E_BYTES = NN * 16;
+    static constexpr uint32_t OFF_KH = EX_BYTES, OFF_TW = OFF_KH + KH_BYTES, OFF_E = OFF_TW + TW_BYTES, OFF_BAR = OFF_E + E_BYTES,
+                              SMEM = OFF_BAR + 16;
+};
+
+template <int N> struct KhHalf {     // K-hat of slot m of a parity block from the stored half
+    const double *blk;               // the block's stored slots
+    int odd;
+    __device__ __forceinline__ double operator()(int m) const { return blk[m <= (N - odd) / 2 ? m : N - odd - m]; }
+};
+
+// every twiddle w_2N^{j (2 k1 + P)} from a shared-memory copy of the table laid out [2 k1 + P][j]
+template <int T> struct TwAllShared {
+    const double2 *base;   // table + j
+    static constexpr bool RECUR = false;
+    template <int P> __device__ __forceinline__ double2 get(int k1) const { return base[(2 * k1 + P) * T]; }
 };
 
 __host__ __device__ __forceinline__ constexpr int freq_to_slot(int k, int N)   // inverse of cmfft::slot_to_freq
@@ -118,6 +136,7 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
     using Lay = LayBatch<T>;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2 *smem = reinterpret_cast<double2 *>(smem_raw);
+    double2 *tw_s = reinterpret_cast<double2 *>(smem_raw + C::OFF_TW), *E_s = reinterpret_cast<double2 *>(smem_raw + C::OFF_E);
     const uint32_t s0 = smem_u32(smem_raw), bar_k = s0 + C::OFF_BAR;
     const int tid = threadIdx.x, px = tid & 7, j = dec_j<T, DEC>((tid >> 3) % T), g = tid / (8 * T), pen = g * 8 + px;
     // CTA -> (fy, group of PEN adjacent sx): fy = 0 .. N (the non-negative y frequencies); the tile at -fy follows
@@ -127,19 +146,27 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
     if (tid == 0) {
         mbar_init(bar_k, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        mbar_expect_tx(bar_k, PEN * NN * 8);
+        mbar_expect_tx(bar_k, PEN * (C::KE + N / 2) * 8);
         const double *ksrc = Kt + ((size_t)sy_a * NN + (size_t)gx * PEN) * C::RSK;
 #pragma unroll 1
-        for (int q = 0; q < PEN; ++q)
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                             s0 + C::OFF_KH + q * (C::RSKS * 8)),
-                         "l"(ksrc + (size_t)q * C::RSK), "r"(NN * 8), "r"(bar_k)
+        for (int q = 0; q < PEN; ++q) {
+            const uint32_t dst = s0 + C::OFF_KH + q * (C::RSKH * 8);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                         "l"(ksrc + (size_t)q * C::RSK), "r"(C::KE * 8), "r"(bar_k)
                          : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst + C::KE * 8),
+                         "l"(ksrc + (size_t)q * C::RSK + N), "r"((N / 2) * 8), "r"(bar_k)
+                         : "memory");
+        }
     }
-    __syncthreads();     // the barrier is initialised before anyone waits on it
-    const double *kh = reinterpret_cast<const double *>(smem_raw + C::OFF_KH) + pen * C::RSKS;
+    // twiddles and E feed multiplies directly: from global memory their latency was 26 % of the warp time (ncu, T = 32)
+    for (int i = tid; i < 32 * T; i += batch_threads<T>()) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
+    for (int i = tid; i < NN; i += batch_threads<T>()) E_s[i] = __ldg(&E[i]);
+    __syncthreads();     // tables in place; the barrier is initialised before anyone waits on it
+    const double *kh_s = reinterpret_cast<const double *>(smem_raw + C::OFF_KH) + pen * C::RSKH;
+    const KhHalf<N> kh0{kh_s, 0}, kh1{kh_s + C::KE, 1};
     double2 *bufA = smem + pen * Lay::PS, *bufB = bufA + PEN * Lay::PS;
-    const TwGlobal twg{tw, j};
+    const TwAllShared<T> twg{tw_s + j};
 
     for (int t = 0; t < ntile; ++t) {
         double2 *col = W2 + ((size_t)(t ? sy_b : sy_a) * NN + (size_t)gx * PEN + pen);
@@ -152,15 +179,15 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
         {
             double2 v[16];
             fwd_half<T, 0, Lay>(a, v, j, bufA, twg, SyncBlock());
-            mul_E<T>(v, E, j);
+            mul_E<T>(v, E_s, j);
             if (t == 0) mbar_wait(bar_k, 0);
-            inv_half<T, 0, Lay, false, true, DEC>(v, e, j, bufB, twg, SyncBlock(), kh);
+            inv_half<T, 0, Lay, false, true, DEC>(v, e, j, bufB, twg, SyncBlock(), kh0);
         }
         {
             double2 v[16];
             fwd_half<T, 1, Lay>(a, v, j, bufA, twg, SyncBlock());
-            mul_E<T>(v, E + N, j);
-            inv_half<T, 1, Lay, false, true, DEC>(v, e, j, bufB, twg, SyncBlock(), kh + N);
+            mul_E<T>(v, E_s + N, j);
+            inv_half<T, 1, Lay, false, true, DEC>(v, e, j, bufB, twg, SyncBlock(), kh1);
         }
         if ((j % DEC) == 0) {
 #pragma unroll

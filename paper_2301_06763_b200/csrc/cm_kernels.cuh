@@ -107,6 +107,10 @@ template <int P, class Tw> __device__ __forceinline__ double2 tw_next(const Tw &
 // ---- half transforms ---------------------------------------------------------------
 // element (row, col) of a pencil's exchange matrix
 template <class Lay> __device__ __forceinline__ double2 &ex_at(double2 *sm, int row, int col) { return sm[row * Lay::RS + col]; }
+// K-hat of a slot: a pencil's parity block as it lies in memory, or an accessor (cm_expand.cuh keeps only the half that
+// the evenness of K-hat in the z frequency leaves)
+__device__ __forceinline__ double kh_at(const double *kh, int slot) { return kh[slot]; }
+template <class KH> __device__ __forceinline__ double kh_at(const KH &kh, int slot) { return kh(slot); }
 
 // Forward, parity P: a[r] = input element n = j + T r (r < 16).  On return
 // v[cc*T + k2] is the spectrum value of slot  P*N + 16*k2 + cc*T + j.
@@ -160,9 +164,8 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
 // kh[16*k2 + cc*T] (K-hat of this thread's slots, Eq. 11), folded into the first butterflies.
 // DEC > 1 (cm_expand.cuh): only the threads with j % DEC == 0 run the last stage — their outputs n = j + T r are the
 // multiples of DEC, all a decimated inverse keeps; the others only take part in the exchange.
-template <int T, int P, class Lay, bool PRE = false, bool KM = false, int DEC = 1, class Sync, class Tw>
-__device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm, Tw tw, Sync sync,
-                                         const double *kh = nullptr)
+template <int T, int P, class Lay, bool PRE = false, bool KM = false, int DEC = 1, class Sync, class Tw, class KH = const double *>
+__device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int j, double2 *sm, Tw tw, Sync sync, KH kh = nullptr)
 {
     static_assert(DEC == 1 || (T > 1 && T % DEC == 0), "decimation needs the radix-T stage");
     double2 w[16];
@@ -174,7 +177,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
                 if (KM) {
                     double k[T];
 #pragma unroll
-                    for (int k2 = 0; k2 < T; ++k2) k[k2] = kh[vslot<T>(cc * T + k2, j)];
+                    for (int k2 = 0; k2 < T; ++k2) k[k2] = kh_at(kh, vslot<T>(cc * T + k2, j));
                     cmfft::DftK<T, +1>::run(&v[cc * T], k);
                 } else {
                     Dft<T, +1>::run(&v[cc * T]);
@@ -192,7 +195,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
                 if (KM) {
 #pragma unroll
                     for (int m = 0; m < 16; ++m) {
-                        const double k = kh[vslot<T>(m, j)];
+                        const double k = kh_at(kh, vslot<T>(m, j));
                         v[m].x *= k;
                         v[m].y *= k;
                     }
@@ -204,7 +207,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
                 if (KM) {
                     double k[16];
 #pragma unroll
-                    for (int m = 0; m < 16; ++m) k[m] = kh[vslot<T>(m, j)];
+                    for (int m = 0; m < 16; ++m) k[m] = kh_at(kh, vslot<T>(m, j));
                     cmfft::DftK<16, +1>::run(v, k);
                 } else {
                     Dft<16, +1>::run(v);
@@ -229,7 +232,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
 #pragma unroll
         for (int k1 = 0; k1 < 16; ++k1) {
             w[k1] = v[k1];
-            if (KM) { w[k1].x *= kh[vslot<T>(k1, j)]; w[k1].y *= kh[vslot<T>(k1, j)]; }
+            if (KM) { const double k = kh_at(kh, vslot<T>(k1, j)); w[k1].x *= k; w[k1].y *= k; }
         }
     }
     if (P) {
