@@ -45,11 +45,13 @@ enum {
 /*
  * Create a plan for `levels` nested N^3 grids.
  *   out        : receives the plan (host pointer to a host pointer).
- *   N          : cells per axis of every level; power of two, 16 <= N <= 512
- *                (N % 4 == 0 is the method's own requirement, L76; N < 16 and N with factors 3 or 5 are
- *                not built: the transform is radix-16 in registers x radix-N/16 across threads).  N = 512
- *                runs the plain P3 kernel (no TMA staging, K-hat from global memory): it exists for the
- *                expanded grids of the modified method and is not tuned like N <= 256.
+ *   N          : cells per axis of every level; N % 4 == 0 (the method's own requirement, L76), 16 <= N <= 512.
+ *                Powers of two are the native sizes.  Any other N runs the same passes at the next power of two
+ *                Nf >= N (a linear convolution needs a transform length of at least 2N - 1, L143; the surplus is more
+ *                zero padding): arrays, rows, planes and the cavity geometry follow N, the spectra and K-hat follow Nf,
+ *                and the cost is about that of Nf.  There are no radix-3 / radix-5 stages (the transform is radix-16
+ *                in registers x radix-Nf/16 across threads), and N = 8 or 12 has no decomposition here.  Nf = 512
+ *                runs the plain P3 kernel (no TMA staging, K-hat from global memory) and is not tuned like Nf <= 256.
  *   levels     : number of nested grids m >= 1 (at most 32).
  *   dx0        : cell size of level 0, > 0; dx_l = dx0 / 2^l (L48).
  *   refinement : must be 2 (the paper fixes the ratio, L42).

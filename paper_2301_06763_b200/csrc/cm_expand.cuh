@@ -48,9 +48,12 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd_blk(const double *__restrict
     using Lay = LayRow<T>;
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
-    const size_t rc = (size_t)blockIdx.x * ROWS + rowl;
+    size_t rc = (size_t)blockIdx.x * ROWS + rowl;
+    const bool valid = rc < (size_t)Nc * Nc;       // the last CTA may be ragged: surplus threads redo the last row, storing nothing
+    if (!valid) rc = (size_t)Nc * Nc - 1;
     const int zc = (int)(rc / Nc), yc = (int)(rc % Nc);
-    double2 *dst = W1 + ((size_t)(c0 + zc) * N + (c0 + yc)) * NN;
+    const int nbig = 2 * c0 + Nc;                  // rows per plane of the expanded grid as W1 holds it
+    double2 *dst = W1 + ((size_t)(c0 + zc) * nbig + (c0 + yc)) * NN;
     double2 a[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
@@ -62,14 +65,18 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd_blk(const double *__restrict
     {
         double2 v[16];
         fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncWarp());
+        if (valid) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) dst[vslot<T>(i, j)] = v[i];
+            for (int i = 0; i < 16; ++i) dst[vslot<T>(i, j)] = v[i];
+        }
     }
     {
         double2 v[16];
         fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, SyncWarp());
+        if (valid) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) dst[N + vslot<T>(i, j)] = v[i];
+            for (int i = 0; i < 16; ++i) dst[N + vslot<T>(i, j)] = v[i];
+        }
     }
 }
 
@@ -84,7 +91,8 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd_blk(const double2 
     const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // zc * 2N + sx
     const size_t z = c0 + q / NN;
     const int sx = (int)(q % NN);
-    y_fwd_body<T>(W1 + z * N * NN + sx, W2 + z * NN * NN + sx, tw, smem, c0, c0 + Nc);
+    const size_t nbig = 2 * (size_t)c0 + Nc;       // rows per plane of the expanded grid as W1 holds it
+    y_fwd_body<T>(W1 + z * nbig * NN + sx, W2 + z * NN * NN + sx, tw, smem, c0, c0 + Nc);
 }
 
 // P3 on an expanded grid, batch-fastest mapping (lane = 8 adjacent pencils x 4 values of j; loads and stores straight
@@ -191,7 +199,8 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
         }
         if ((j % DEC) == 0) {
 #pragma unroll
-            for (int r = 0; r < 16; ++r) col[(size_t)((j + T * r) / DEC) * ZS] = e[r];
+            for (int r = 0; r < 16; ++r)
+                if ((j + T * r) / DEC < zhi - zlo) col[(size_t)((j + T * r) / DEC) * ZS] = e[r];    // the Nc coarse planes
         }
     }
 }
@@ -199,7 +208,7 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
 // P4, decimated: plane bz = coarse z; the N / DEC coarse rows a = (j + T r) / DEC of W1 (plane stride as in the plain pass).
 template <int T, int DEC>
 __global__ void __launch_bounds__(batch_threads<T>()) k_y_inv_dec(const double2 *__restrict__ W2, double2 *__restrict__ W1,
-                                                                  const double2 *__restrict__ tw, const double2 *__restrict__ E)
+                                                                  const double2 *__restrict__ tw, const double2 *__restrict__ E, int Nc)
 {
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     using Lay = LayBatch<T>;
@@ -223,22 +232,25 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_inv_dec(const double2 
     inv_half<T, 1, Lay, false, false, DEC>(v1, e, j, bufB, TwGlobal{tw, j}, SyncBlock());
     if ((j % DEC) == 0) {
 #pragma unroll
-        for (int r = 0; r < 16; ++r) dst[(size_t)((j + T * r) / DEC) * NN] = e[r];
+        for (int r = 0; r < 16; ++r)
+            if ((j + T * r) / DEC < Nc) dst[(size_t)((j + T * r) / DEC) * NN] = e[r];
     }
 }
 
-// P5, decimated: compact row rc = az Nc + ay (Nc = N / DEC) of W1 -> the Nc block sums along x, times `scale`;
+// P5, decimated: compact row rc = az Nc + ay (Nc coarse cells per axis) of W1 -> the Nc block sums along x, times `scale`;
 // real part to out_re, imaginary part (the second field) to out_im if given.  Compact Nc^3 outputs.
 template <int T, int DEC>
 __global__ void __launch_bounds__(kThreads) k_x_inv_dec(const double2 *__restrict__ W1, double *__restrict__ out_re,
                                                         double *__restrict__ out_im, const double2 *__restrict__ tw,
-                                                        const double2 *__restrict__ E, double scale)
+                                                        const double2 *__restrict__ E, double scale, int Nc)
 {
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, Nc = N / DEC;
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T;
     using Lay = LayRow<T>;
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
-    const size_t rc = (size_t)blockIdx.x * ROWS + rowl;
+    size_t rc = (size_t)blockIdx.x * ROWS + rowl;
+    const bool valid = rc < (size_t)Nc * Nc;
+    if (!valid) rc = (size_t)Nc * Nc - 1;
     const size_t az = rc / Nc, ay = rc % Nc;
     const double2 *src = W1 + (az * N + ay) * NN;
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
@@ -252,9 +264,10 @@ __global__ void __launch_bounds__(kThreads) k_x_inv_dec(const double2 *__restric
     mul_E<T>(v1, E + N, j);
     inv_half<T, 0, Lay, false, false, DEC>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
     inv_half<T, 1, Lay, false, false, DEC>(v1, e, j, bufB, TwGlobal{tw, j}, SyncWarp());
-    if ((j % DEC) == 0) {
+    if (valid && (j % DEC) == 0) {
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
+            if ((j + T * r) / DEC >= Nc) continue;
             const size_t o = rc * Nc + (j + T * r) / DEC;
             out_re[o] = scale * e[r].x;
             if (out_im) out_im[o] = scale * e[r].y;

@@ -251,52 +251,65 @@ __device__ __forceinline__ bool in_ring1(int v, int N) { return v >= N / 4 - 1 &
 // One row (b, z, y) per group of T threads (j fastest).  Reads N reals, forms the complex
 // pair field (step a2, never materialised), writes 2N complex slots.
 // body: thread (rowl, j) of a CTA transforms global row `row` (b, z, y) and writes its 2N slots to `dst`
-template <int T>
+// GEN (general sizes): the level has nd <= N cells per axis (nd % 4 == 0) and is transformed at the next power
+// of two N = 16 T — the rows, the cavity geometry and the arrays of the caller follow nd, the spectra follow N; cells
+// x >= nd are zero like the padding.  GEN = false: nd = N at compile time (the code of the power-of-two sizes).
+template <int T, bool GEN = false>
 __device__ __forceinline__ void x_fwd_body(const double *__restrict__ rho, const double *__restrict__ rc, double2 *dst,
-                                           const double2 *__restrict__ tw, int L, size_t row, double2 *smem)
+                                           const double2 *__restrict__ tw, int L, size_t row, double2 *smem, int nd_arg = 0,
+                                           bool valid = true)
 {
-    constexpr int N = 16 * T, ROWS = kThreads / T, H = N / 2, Q = N / 4;
+    constexpr int N = 16 * T, ROWS = kThreads / T;
+    const int nd = GEN ? nd_arg : N, H = nd / 2, Q = nd / 4;
     using Lay = LayRow<T>;
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
-    const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
+    const int y = (int)(row % nd), z = (int)((row / nd) % nd), b = (int)(row / ((size_t)nd * nd));
     const bool finest = (b == L - 1);
-    const bool rowcav = !finest && in_cavity1(z, N) && in_cavity1(y, N);
-    const double *src = rho + row * N;
+    const bool rowcav = !finest && in_cavity1(z, nd) && in_cavity1(y, nd);
+    const double *src = rho + row * nd;
     const double *srcc = rowcav ? rc + (((size_t)b * H + (z - Q)) * H + (y - Q)) * H - Q : rho;
 
     double2 a[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
         const int x = j + T * r;
-        const bool cav = rowcav && in_cavity1(x, N);
-        const double re = cav ? __ldg(srcc + x) : __ldg(src + x);
+        const bool cav = rowcav && in_cavity1(x, nd);
+        double re = 0.0;
+        if (!GEN || x < nd) re = cav ? __ldg(srcc + x) : __ldg(src + x);
         a[r] = make_double2(re, (finest || cav) ? 0.0 : re);
     }
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
     {
         double2 v[16];
         fwd_half<T, 0, Lay>(a, v, j, bufA, TwGlobal{tw, j}, SyncWarp());
+        if (!GEN || valid) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) dst[vslot<T>(i, j)] = v[i];
+            for (int i = 0; i < 16; ++i) dst[vslot<T>(i, j)] = v[i];
+        }
     }
     {
         double2 v[16];
         fwd_half<T, 1, Lay>(a, v, j, bufB, TwGlobal{tw, j}, SyncWarp());
+        if (!GEN || valid) {
 #pragma unroll
-        for (int i = 0; i < 16; ++i) dst[N + vslot<T>(i, j)] = v[i];
+            for (int i = 0; i < 16; ++i) dst[N + vslot<T>(i, j)] = v[i];
+        }
     }
 }
 
-template <int T>
+template <int T, bool GEN = false>
 __global__ void __launch_bounds__(kThreads) k_x_fwd(const double *__restrict__ rho, const double *__restrict__ rc,
                                                     double2 *__restrict__ W1, const double2 *__restrict__ tw, int L,
-                                                    size_t row0)
+                                                    size_t row0, int nd = 0, size_t row_end = 0)
 {
-    // row0: first global row (b, z, y) of this launch
+    // row0: first global row (b, z, y) of this launch; GEN: rows at and beyond row_end do not exist (the last CTA is ragged:
+    // its surplus threads redo the last row without storing, so that every warp stays whole for the exchanges)
     constexpr int NN = 32 * T, ROWS = kThreads / T;
     extern __shared__ double2 smem[];
-    const size_t row = row0 + (size_t)blockIdx.x * ROWS + threadIdx.x / T;
-    x_fwd_body<T>(rho, rc, W1 + row * NN, tw, L, row, smem);
+    size_t row = row0 + (size_t)blockIdx.x * ROWS + threadIdx.x / T;
+    const bool valid = !GEN || row < row_end;
+    if (GEN && !valid) row = row_end - 1;
+    x_fwd_body<T, GEN>(rho, rc, W1 + row * NN, tw, L, row, smem, nd, valid);
 }
 
 // P1 split by output parity (see k_y_fwd_split): 256 threads, warps 0-3 the even slots, warps 4-7 the odd ones
@@ -353,20 +366,25 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 // LATE (N <= 128): fetch Hc after the transforms, behind griddepcontrol.wait — the level overlaps the one before it.
 // N = 256 (a level is 28 waves, the overlap is worth little): wait first and fetch Hc at the top, so that its latency
 // hides behind the transforms as before (measured: late fetch there 1.68 -> 2.18 ms).
-template <int T>
+template <int T, bool GEN = false>
 __global__ void __launch_bounds__(kThreads, 2) k_x_inv(const double2 *__restrict__ W1, double *__restrict__ phi,
                                                     double *__restrict__ hole, const double *__restrict__ hole_c,
                                                     const double2 *__restrict__ tw, int L, double scale0 /* -G dx0^2 */,
-                                                    size_t row0, int hole_all)
+                                                    size_t row0, int hole_all, int nd_arg = 0)
 {
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, Q = N / 4;
+    // GEN: nd <= N cells per axis (see x_fwd_body); a level has nd^2 rows, the last CTA may be ragged
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T;
+    const int nd = GEN ? nd_arg : N, Q = nd / 4;
     constexpr bool LATE = (T <= 8);
     using Lay = LayRow<T>;
     extern __shared__ double2 smem[];
     pdl_launch_dependents();
     const int tid = threadIdx.x, j = tid % T, rowl = tid / T;
-    const size_t rowc = (size_t)blockIdx.x * ROWS + rowl, row = row0 + rowc;
-    const int y = (int)(row % N), z = (int)((row / N) % N), b = (int)(row / ((size_t)N * N));
+    size_t rowc = (size_t)blockIdx.x * ROWS + rowl;
+    const bool valid = !GEN || rowc < (size_t)nd * nd;
+    if (GEN && !valid) rowc = (size_t)nd * nd - 1;
+    const size_t row = row0 + rowc;
+    const int y = (int)(row % nd), z = (int)((row / nd) % nd), b = (int)(row / ((size_t)nd * nd));
     const double2 *src = W1 + row * NN;
     double2 *bufA = smem + rowl * Lay::PS, *bufB = bufA + ROWS * Lay::PS;
 
@@ -375,13 +393,13 @@ __global__ void __launch_bounds__(kThreads, 2) k_x_inv(const double2 *__restrict
     auto fetch_ext = [&]() {
         if (b > 0) {
             pdl_wait();
-            const double *Hc = hole_c + (size_t)(b - 1) * N * N * N;
+            const double *Hc = hole_c + (size_t)(b - 1) * nd * nd * nd;
             const int pk = Q + z / 2, pj = Q + y / 2, sk = (z & 1) ? 1 : -1, sj = (y & 1) ? 1 : -1;
-            const double *h0 = Hc + ((size_t)pk * N + pj) * N, *h1 = Hc + ((size_t)(pk + sk) * N + (pj + sj)) * N;
+            const double *h0 = Hc + ((size_t)pk * nd + pj) * nd, *h1 = Hc + ((size_t)(pk + sk) * nd + (pj + sj)) * nd;
 #pragma unroll
             for (int r = 0; r < 16; ++r) {
                 const int x = j + T * r, pi = Q + x / 2, si = (x & 1) ? 1 : -1;
-                ext[r] = 0.75 * __ldcg(h0 + pi) + 0.25 * __ldcg(h1 + pi + si);
+                ext[r] = (!GEN || x < nd) ? 0.75 * __ldcg(h0 + pi) + 0.25 * __ldcg(h1 + pi + si) : 0.0;
             }
         } else {
 #pragma unroll
@@ -400,16 +418,18 @@ __global__ void __launch_bounds__(kThreads, 2) k_x_inv(const double2 *__restrict
     inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncWarp());
     inv_half<T, 1, Lay>(v1, e, j, bufB, TwGlobal{tw, j}, SyncWarp());     // adds the odd half
     if (LATE) fetch_ext();
+    if (GEN && !valid) return;
 
-    const bool rowring = (b < L - 1) && in_ring1(z, N) && in_ring1(y, N);
+    const bool rowring = (b < L - 1) && in_ring1(z, nd) && in_ring1(y, nd);
     const double scale = scale0 * exp2(-2.0 * b);   // dx_b^2 = dx0^2 / 4^b, exact
-    double *dphi = phi + row * N, *dh = hole + row * N;
+    double *dphi = phi + row * nd, *dh = hole + row * nd;
 #pragma unroll
     for (int r = 0; r < 16; ++r) {
         const int x = j + T * r;
+        if (GEN && x >= nd) continue;
         const double re = scale * e[r].x, im = scale * e[r].y;
         dphi[x] = b > 0 ? re + ext[r] : re;
-        if (hole_all ? (b < L - 1) : (rowring && in_ring1(x, N))) dh[x] = b > 0 ? im + ext[r] : im;
+        if (hole_all ? (b < L - 1) : (rowring && in_ring1(x, nd))) dh[x] = b > 0 ? im + ext[r] : im;
     }
 }
 
@@ -453,17 +473,19 @@ __device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, con
     }
 }
 
-template <int T>
+template <int T, bool GEN = false>
 __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd(const double2 *__restrict__ W1, double2 *__restrict__ W2,
-                                                    const double2 *__restrict__ tw)
+                                                    const double2 *__restrict__ tw, int nd_arg = 0)
 {
+    // GEN: a plane has nd <= N rows of data (see x_fwd_body); bz counts the nd planes of every level
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
+    const int nd = GEN ? nd_arg : N;
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, px = tid & 7, g = tid / (8 * T);
-    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*N + z) * 2N + sx
+    const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*nd + z) * 2N + sx
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
-    y_fwd_body<T>(W1 + bz * N * NN + sx, W2 + bz * NN * NN + sx, tw, smem);
+    y_fwd_body<T>(W1 + bz * nd * NN + sx, W2 + bz * NN * NN + sx, tw, smem, 0, nd);
 }
 
 // P2 split by output parity: 256 threads, warps 0-3 form the even slots (P = 0), warps 4-7 the odd ones
@@ -499,11 +521,13 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *
 }
 
 // ================================ P4: y inverse ====================================
-template <int T>
+template <int T, bool GEN = false>
 __global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
-                                                    const double2 *__restrict__ tw)
+                                                    const double2 *__restrict__ tw, int nd_arg = 0)
 {
+    // GEN: only the nd <= N rows of data are kept (see x_fwd_body)
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
+    const int nd = GEN ? nd_arg : N;
     using Lay = LayBatch<T>;
     extern __shared__ double2 smem[];
     const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T);
@@ -511,7 +535,7 @@ __global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(c
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
     const double2 *src = W2 + bz * NN * NN + sx;
-    double2 *dst = W1 + bz * N * NN + sx;
+    double2 *dst = W1 + bz * nd * NN + sx;
     double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
 
     double2 v0[16], v1[16];
@@ -524,7 +548,8 @@ __global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(c
     inv_half<T, 0, Lay>(v0, e, j, bufA, TwGlobal{tw, j}, SyncBlock());
     inv_half<T, 1, Lay>(v1, e, j, bufB, TwGlobal{tw, j}, SyncBlock());   // adds the odd half
 #pragma unroll
-    for (int r = 0; r < 16; ++r) dst[(size_t)(j + T * r) * NN] = e[r];
+    for (int r = 0; r < 16; ++r)
+        if (!GEN || j + T * r < nd) dst[(size_t)(j + T * r) * NN] = e[r];
 }
 
 // ============================ a1: restriction cascade ==============================

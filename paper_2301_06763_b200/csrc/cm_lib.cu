@@ -27,7 +27,9 @@ constexpr size_t kGraphCacheSize = 8;
 }  // namespace
 
 struct cm_plan {
-    int N = 0, L = 0, T = 0;
+    int N = 0, L = 0, T = 0;       // N: cells per axis of a level; the transforms run at Nf = 16 T = the next power of two >= N
+    int Nf = 0;
+    bool gen = false;               // N < Nf: the general-size instantiations of the passes
     double dx0 = 0, G = 1.0;
     double2 *W1 = nullptr, *W2 = nullptr, *tw = nullptr;
     double *Khat = nullptr, *rc = nullptr, *hole = nullptr, *pbar = nullptr;
@@ -72,10 +74,16 @@ template <int T> size_t smem_batch() { return sizeof(double2) * 2 * batch_pencil
 
 template <int T> int set_attrs(cm_plan *p)
 {
-    CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-    CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    if constexpr (T >= 2) {     // general sizes (N < 16 T)
+        CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    }
     if constexpr (T <= 16) {
         CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
         CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
@@ -103,10 +111,10 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
                 return;
             }
         }
-        k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0);
+        k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0, p->N);
     } else {
         const unsigned ngroups = (unsigned)(NN * NN / batch_pencils<T>());
-        k_z_conv_batch<T><<<ngroups * (unsigned)L, batch_threads<T>(), smem_batch<T>(), s>>>(p->Khat, p->W2, p->tw, b0);
+        k_z_conv_batch<T><<<ngroups * (unsigned)L, batch_threads<T>(), smem_batch<T>(), s>>>(p->Khat, p->W2, p->tw, b0, p->N);
     }
 }
 
@@ -116,7 +124,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
 template <int T>
 void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid, double scale0, bool chained, int hole_all)
 {
-    constexpr int N = 16 * T;
+    const size_t nd = (size_t)p->N;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(kThreads);
@@ -127,8 +135,12 @@ void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid,
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = chained ? 1 : 0;
-    cudaLaunchKernelEx(&cfg, k_x_inv<T>, (const double2 *)p->W1, phi, p->hole, (const double *)p->hole, (const double2 *)p->tw, p->L,
-                       scale0, (size_t)b * N * N, hole_all);
+    if (p->gen)
+        cudaLaunchKernelEx(&cfg, k_x_inv<T, true>, (const double2 *)p->W1, phi, p->hole, (const double *)p->hole, (const double2 *)p->tw,
+                           p->L, scale0, (size_t)b * nd * nd, hole_all, p->N);
+    else
+        cudaLaunchKernelEx(&cfg, k_x_inv<T, false>, (const double2 *)p->W1, phi, p->hole, (const double *)p->hole, (const double2 *)p->tw,
+                           p->L, scale0, (size_t)b * nd * nd, hole_all, p->N);
 }
 
 // The five FFT passes (steps a3-a7) with the prolongation + Eq. 14 sum (a8) folded into P5:
@@ -137,31 +149,39 @@ void launch_x_inv(cm_plan *p, double *phi, cudaStream_t s, int b, unsigned grid,
 template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev, int hole_all)
 {
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
-    const int L = p->L;
-    const size_t planes = (size_t)L * N;
+    const int L = p->L, nd = p->N;
+    const size_t planes = (size_t)L * nd, rows = planes * nd;
     const double scale0 = -p->G * p->dx0 * p->dx0;
+    const unsigned gx = (unsigned)((rows + ROWS - 1) / ROWS), gy = (unsigned)(planes * NN / PEN);
     bool done_x = false, done_y = false;
     if constexpr (T <= 16) {
         if (p->split_x) {
-            k_x_fwd_split<T><<<(unsigned)(planes * N / ROWS), 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
+            k_x_fwd_split<T><<<gx, 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
             done_x = true;
         }
     }
-    if (!done_x) k_x_fwd<T><<<(unsigned)(planes * N / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
+    if (!done_x) {
+        if (p->gen) k_x_fwd<T, true><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0, nd, rows);
+        else k_x_fwd<T, false><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L, 0);
+    }
     if (ev) cudaEventRecord(ev[2], s);
     if constexpr (T <= 16) {
         if (p->split_y) {
-            k_y_fwd_split<T><<<(unsigned)(planes * NN / PEN), 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+            k_y_fwd_split<T><<<gy, 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
             done_y = true;
         }
     }
-    if (!done_y) k_y_fwd<T><<<(unsigned)(planes * NN / PEN), BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    if (!done_y) {
+        if (p->gen) k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, nd);
+        else k_y_fwd<T, false><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+    }
     if (ev) cudaEventRecord(ev[3], s);
     launch_zconv<T>(p, s, 0, L);
     if (ev) cudaEventRecord(ev[4], s);
-    k_y_inv<T><<<(unsigned)(planes * NN / PEN), BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
+    if (p->gen) k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw, nd);
+    else k_y_inv<T, false><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
     if (ev) cudaEventRecord(ev[5], s);
-    const size_t lrows = (size_t)N * N;
+    const size_t lrows = (size_t)nd * nd;
     const unsigned gl = (unsigned)((lrows + ROWS - 1) / ROWS);
     for (int b = 0; b < L; ++b) launch_x_inv<T>(p, phi, s, b, gl, scale0, /*chained=*/b > 0, hole_all);
     if (ev) cudaEventRecord(ev[6], s);
@@ -176,17 +196,26 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
 template <int T> void level_p1_to_p4(cm_plan *p, const double *rho, cudaStream_t s, int l)
 {
     constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
-    const size_t lrows = (size_t)N * N;
-    double2 *w1 = p->W1 + (size_t)l * lrows * NN, *w2 = p->W2 + (size_t)l * N * NN * NN;
-    k_x_fwd<T><<<(unsigned)(lrows / ROWS), kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows);
-    k_y_fwd<T><<<(unsigned)((size_t)N * NN / PEN), BT, smem_batch<T>(), s>>>(w1, w2, p->tw);
-    launch_zconv<T>(p, s, l, 1);
-    k_y_inv<T><<<(unsigned)((size_t)N * NN / PEN), BT, smem_batch<T>(), s>>>(w2, w1, p->tw);
+    const int nd = p->N;
+    const size_t lrows = (size_t)nd * nd;
+    double2 *w1 = p->W1 + (size_t)l * lrows * NN, *w2 = p->W2 + (size_t)l * nd * NN * NN;
+    const unsigned gx = (unsigned)((lrows + ROWS - 1) / ROWS), gy = (unsigned)((size_t)nd * NN / PEN);
+    if (p->gen) {
+        k_x_fwd<T, true><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows, nd, (size_t)(l + 1) * lrows);
+        k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw, nd);
+        launch_zconv<T>(p, s, l, 1);
+        k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw, nd);
+    } else {
+        k_x_fwd<T, false><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)l * lrows);
+        k_y_fwd<T, false><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw);
+        launch_zconv<T>(p, s, l, 1);
+        k_y_inv<T, false><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw);
+    }
 }
 template <int T> void level_p5(cm_plan *p, double *phi, cudaStream_t s, int l)
 {
-    constexpr int N = 16 * T, ROWS = kThreads / T;
-    const size_t lrows = (size_t)N * N;
+    constexpr int ROWS = kThreads / T;
+    const size_t lrows = (size_t)p->N * p->N;
     launch_x_inv<T>(p, phi, s, l, (unsigned)((lrows + ROWS - 1) / ROWS), -p->G * p->dx0 * p->dx0, /*chained=*/false, 0);
 }
 void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int l, bool p5)
@@ -270,9 +299,9 @@ int make_tensor_maps(cm_plan *p)
         return CM_ECUDA;
     }
     EncodeTiledFn enc = (EncodeTiledFn)fn;
-    const cuuint64_t NN = 2 * (cuuint64_t)p->N, N = p->N, L = p->L;
+    const cuuint64_t NN = 2 * (cuuint64_t)p->Nf, N = p->N, L = p->L;     // N rows of data per level, spectra of 2 Nf slots
     const cuuint32_t es[2] = {1, 1};
-    {   // W2 as fp64 [L*N rows][2*(2N)^2]; box = 16 doubles (8 complex = 128 B) x N rows, 128B swizzle
+    {   // W2 as fp64 [L*N rows][2*(2Nf)^2]; box = 16 doubles (8 complex = 128 B) x N rows, 128B swizzle
         const cuuint64_t dims[2] = {2 * NN * NN, L * N};
         const cuuint64_t strides[1] = {NN * NN * 16};
         const cuuint32_t box[2] = {16, (cuuint32_t)N};
@@ -284,7 +313,7 @@ int make_tensor_maps(cm_plan *p)
             return CM_ECUDA;
         }
     }
-    if (p->N >= 128) {   // per-warp boxes: PPW pencils (32 B at N = 256, 64 B at N = 128) x N rows, swizzle = the row width
+    if (p->N >= 128 && !p->gen) {   // per-warp boxes: PPW pencils (32 B at N = 256, 64 B at N = 128) x N rows, swizzle = the row width
         const int ppw = 32 / (p->N / 16);
         const cuuint64_t dims[2] = {2 * NN * NN, L * N};
         const cuuint64_t strides[1] = {NN * NN * 16};
@@ -350,7 +379,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
     if (!out) return CM_EINVAL;
     *out = nullptr;
     if (refinement != 2) return CM_EINVAL;
-    if (N < 16 || N > 512 || (N & (N - 1)) != 0) return CM_EINVAL;
+    if (N < 16 || N > 512 || (N % 4) != 0) return CM_EINVAL;
     if (levels < 1 || levels > 32) return CM_EINVAL;
     if (!(dx0 > 0.0) || !std::isfinite(dx0)) return CM_EINVAL;
 
@@ -358,7 +387,10 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
     if (!p) return CM_ENOMEM;
     p->N = N;
     p->L = levels;
-    p->T = N / 16;
+    p->Nf = 16;
+    while (p->Nf < N) p->Nf *= 2;       // the transforms run at the next power of two: 2 Nf >= 2 N - 1 is all a linear
+    p->T = p->Nf / 16;                  // convolution needs (L143); the surplus is more zero padding
+    p->gen = (p->Nf != N);
     p->dx0 = dx0;
     // the one environment switch (cm.h): CM_DEBUG=nograph launches kernel by kernel instead of through a CUDA graph
     if (const char *dbg = std::getenv("CM_DEBUG")) {
@@ -368,16 +400,16 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
             return CM_EINVAL;
         }
     }
-    const size_t n = 2 * (size_t)N, n3 = (size_t)N * N * N, h3 = n3 / 8, L = (size_t)levels;
+    const size_t n = 2 * (size_t)p->Nf, n3 = (size_t)N * N * N, h3 = n3 / 8, L = (size_t)levels;
     int rc = CM_OK;
     if ((rc = dev_alloc(p, &p->W1, L * N * N * n)) == CM_OK &&
         (rc = dev_alloc(p, &p->W2, L * N * n * n)) == CM_OK &&
-        (rc = dev_alloc(p, &p->Khat, n * n * (size_t)khat_row_stride(N))) == CM_OK &&
+        (rc = dev_alloc(p, &p->Khat, n * n * (size_t)khat_row_stride(p->Nf))) == CM_OK &&
         (rc = dev_alloc(p, &p->rc, (L > 1 ? L - 1 : 1) * h3)) == CM_OK &&
         (rc = dev_alloc(p, &p->hole, L * n3)) == CM_OK &&
         (rc = dev_alloc(p, &p->pbar, (L > 1 ? L - 1 : 1) * h3)) == CM_OK &&
         (rc = dev_alloc(p, &p->tw, n)) == CM_OK) {
-        // twiddles w_2N^m = exp(-2 pi i m / 2N), computed in long double on the host
+    // twiddles w_2N^m = exp(-2 pi i m / 2N), computed in long double on the host
         std::vector<double2> tw(n);
         const long double tau = 2.0L * acosl(-1.0L);
         for (size_t m = 0; m < n; ++m) {
@@ -404,7 +436,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         if (cuda_fail(p, cudaGetDevice(&dev), "cudaGetDevice") ||
             cuda_fail(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
             rc = CM_ECUDA;
-        else if (N <= 256) rc = make_tensor_maps(p);   // the TMA-fed P3 (N = 512 runs k_z_conv_batch)
+        else if (p->Nf <= 256) rc = make_tensor_maps(p);   // the TMA-fed P3 (Nf = 512 runs k_z_conv_batch)
     }
     if (rc == CM_OK) {
         switch (p->T) {
@@ -431,7 +463,7 @@ int cm_green_precompute(cm_plan *p)
 {
     if (!p) return CM_EINVAL;
     if (p->green_ready) return CM_OK;
-    const int N = p->N, n = 2 * N;
+    const int N = p->Nf, n = 2 * N;          // K-hat of the transform size (a superset of the offsets a level of p->N cells needs)
     const size_t tot = (size_t)n * n * n;
     double2 *Gm = nullptr;
     cudaError_t e = cudaMalloc((void **)&Gm, tot * sizeof(double2));
@@ -554,8 +586,7 @@ namespace {
 template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, const double *src_im, double *out_re, double *out_im,
                                             cudaStream_t s, bool attrs_only)
 {
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>(), Nc = N / F,
-                  c0 = (N - Nc) / 2;
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
     static bool attrs = false;      // per instantiation; the attribute is per function, not per plan
     if (!attrs) {
         CM_CUDA(pe, cudaFuncSetAttribute(k_x_fwd_blk<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
@@ -566,11 +597,14 @@ template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, c
         attrs = true;
     }
     if (attrs_only) return CM_OK;
-    k_x_fwd_blk<T><<<(unsigned)(Nc * Nc / ROWS), kThreads, smem_row<T>(), s>>>(src_re, src_im, pe->W1, pe->tw, Nc, c0);
+    // the expanded grid has pe->N = F Nc cells per axis (transformed at N = 16 T >= pe->N); the block sits in its middle
+    const int Nc = pe->N / F, c0 = (pe->N - Nc) / 2;
+    const unsigned gr = (unsigned)(((size_t)Nc * Nc + ROWS - 1) / ROWS);
+    k_x_fwd_blk<T><<<gr, kThreads, smem_row<T>(), s>>>(src_re, src_im, pe->W1, pe->tw, Nc, c0);
     k_y_fwd_blk<T><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W1, pe->W2, pe->tw, Nc, c0);
     k_z_conv_dec<T, F><<<(unsigned)((size_t)(N + 1) * (NN / PEN)), BT, ZDecCfg<T>::SMEM, s>>>(pe->Khat, pe->W2, pe->tw, pe->decE, c0, c0 + Nc);
-    k_y_inv_dec<T, F><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W2, pe->W1, pe->tw, pe->decE);
-    k_x_inv_dec<T, F><<<(unsigned)(Nc * Nc / ROWS), kThreads, smem_row<T>(), s>>>(pe->W1, out_re, out_im, pe->tw, pe->decE, -1.0);
+    k_y_inv_dec<T, F><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W2, pe->W1, pe->tw, pe->decE, Nc);
+    k_x_inv_dec<T, F><<<gr, kThreads, smem_row<T>(), s>>>(pe->W1, out_re, out_im, pe->tw, pe->decE, -1.0, Nc);
     CM_CUDA(pe, cudaGetLastError());
     return CM_OK;
 }
@@ -598,13 +632,13 @@ int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **src, double **re
     if (rc == CM_OK) rc = cm_green_precompute(*plan);
     if (rc == CM_OK && !(*plan)->decE) {
         cm_plan *pe = *plan;
-        const int n = 2 * pe->N;
+        const int n = 2 * pe->Nf;           // the transform length
         rc = dev_alloc(pe, &pe->decE, (size_t)n);
         if (rc == CM_OK) {
             std::vector<double2> E(n);
             const long double tau = 2.0L * acosl(-1.0L);
             for (int sl = 0; sl < n; ++sl) {
-                const int k = cmfft::slot_to_freq(sl, pe->N);
+                const int k = cmfft::slot_to_freq(sl, pe->Nf);
                 long double re = 0, im = 0;
                 for (int q = 0; q < F; ++q) {
                     const long double a = tau * (long double)(((long long)k * q) % n) / (long double)n;
@@ -803,8 +837,14 @@ int cm_acceleration(cm_plan *p, const double *phi, double *g, void *stream)
         k_child_mean<<<(unsigned)((cnt + 255) / 256), 256, 0, s>>>(p->N, p->L, phi, p->pbar);
     }
     {
-        const int N = p->N, TX = N / 2 < 32 ? N / 2 : 32, TY = (256 / TX) < N ? 256 / TX : N;
-        const int ZCH = N >= 256 ? 16 : (N >= 128 ? 8 : (N >= 64 ? 4 : 2));   // planes a thread marches: enough CTAs at small N
+        // a CTA is a TX x TY tile of cell pairs marching ZCH planes; all three must divide the grid (any N % 4 == 0)
+        auto divisor_le = [](int n, int cap) {
+            int d = cap < n ? cap : n;
+            while (n % d) --d;
+            return d;
+        };
+        const int N = p->N, TX = divisor_le(N / 2, 32), TY = divisor_le(N, 256 / TX);
+        const int ZCH = divisor_le(N, N >= 256 ? 16 : (N >= 128 ? 8 : (N >= 64 ? 4 : 2)));   // planes a thread marches: enough CTAs at small N
         const unsigned grid = (unsigned)((size_t)p->L * (N / ZCH) * (N / TY) * ((N / 2) / TX));
         k_accel<<<grid, TX * TY, 0, s>>>(N, p->L, TX, TY, ZCH, p->dx0, phi, p->pbar, g);
     }
@@ -863,8 +903,8 @@ int cm_debug_copy(cm_plan *p, int which, double *dst, size_t n_doubles, void *st
         case CM_BUF_RESTRICTED: src = p->rc; cnt = (L - 1) * (n3 / 8); break;
         case CM_BUF_HOLE: src = p->hole; cnt = L * n3; break;
         case CM_BUF_KHAT:
-            if (n_doubles != 8 * n3) return CM_EINVAL;
-            k_khat_export<<<1024, 256, 0, (cudaStream_t)stream>>>(p->Khat, dst, p->N);
+            if (n_doubles != 8 * (size_t)p->Nf * p->Nf * p->Nf) return CM_EINVAL;   // K-hat is that of the transform size
+            k_khat_export<<<1024, 256, 0, (cudaStream_t)stream>>>(p->Khat, dst, p->Nf);
             CM_CUDA(p, cudaGetLastError());
             return CM_OK;
         default: return CM_EINVAL;

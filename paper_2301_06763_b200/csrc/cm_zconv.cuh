@@ -97,8 +97,10 @@ template <int T> struct ZConvCfg {
 template <int T>
 __global__ void __launch_bounds__(kThreads, ZConvCfg<T>::CTAS)
 k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict__ Kt,
-             double2 *__restrict__ W2, const double2 *__restrict__ tw, int L, int ngroups, int b0)
+             double2 *__restrict__ W2, const double2 *__restrict__ tw, int L, int ngroups, int b0, int nd)
 {
+    // nd <= N: z-rows of data per level (general sizes): the boxes of mapW are nd rows high, the rows
+    // nd .. N-1 of the input stage are zeroed once and never written again
     using C = ZConvCfg<T>;
     constexpr int N = C::N, PEN = C::PEN, NBOX = C::NBOX;
     using Lay = LayRow<T>;
@@ -142,10 +144,10 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
         // the async-proxy write.  Without this fence the refill raced with them (measured: wrong
         // results whenever two CTAs shared an SM).
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        mbar_expect_tx(bar_in, C::IN_BYTES);
+        mbar_expect_tx(bar_in, (uint32_t)(NBOX * nd * 128));
 #pragma unroll
         for (int q = 0; q < NBOX; ++q)
-            tma_load_2d(s0 + C::OFF_IN + q * (N * 128), &mapW, 2 * (g * PEN + 8 * q), (b0 + b) * N, bar_in);
+            tma_load_2d(s0 + C::OFF_IN + q * (N * 128), &mapW, 2 * (g * PEN + 8 * q), (b0 + b) * nd, bar_in);
     };
     auto issue_k = [&](int g) {
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -162,6 +164,11 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int i = tid; i < 32 * T; i += kThreads) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
+    if (nd < N) {
+        const int tail16 = (N - nd) * 8;       // 16-byte words of the rows nd .. N-1 of one box
+        for (int i = tid; i < NBOX * tail16; i += kThreads)
+            *reinterpret_cast<double2 *>(sbase + C::OFF_IN + (i / tail16) * (N * 128) + nd * 128 + (i % tail16) * 16) = make_double2(0.0, 0.0);
+    }
     __syncthreads();
     if (tid == 0) {
         int g0, b0;
@@ -226,7 +233,7 @@ k_z_conv_tma(const __grid_constant__ CUtensorMap mapW, const double *__restrict_
         if (tid == 0) {
 #pragma unroll
             for (int q = 0; q < NBOX; ++q)
-                tma_store_2d(&mapW, 2 * (g * PEN + 8 * q), (b0 + b) * N, s0 + C::OFF_EX + q * (N * 128));
+                tma_store_2d(&mapW, 2 * (g * PEN + 8 * q), (b0 + b) * nd, s0 + C::OFF_EX + q * (N * 128));
             tma_store_commit();
         }
     }
@@ -385,8 +392,9 @@ k_z_conv_warp(const __grid_constant__ CUtensorMap mapWw, const double *__restric
 // from/to registers in whole 128-byte lines, K-hat read from global memory, two exchange buffers used in turn.
 template <int T>
 __global__ void __launch_bounds__(batch_threads<T>(), 1)
-k_z_conv_batch(const double *__restrict__ Kt, double2 *__restrict__ W2, const double2 *__restrict__ tw, int b0)
+k_z_conv_batch(const double *__restrict__ Kt, double2 *__restrict__ W2, const double2 *__restrict__ tw, int b0, int nd)
 {
+    // nd <= N: z-rows of data per level (general sizes); rows beyond are zero on the way in and not written on the way out
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>(), RSK = khat_row_stride(N);
     constexpr size_t ZS = (size_t)NN * NN;           // stride of z in W2 (complex elements)
     using Lay = LayBatch<T>;
@@ -395,14 +403,14 @@ k_z_conv_batch(const double *__restrict__ Kt, double2 *__restrict__ W2, const do
     const int ngroups = NN * NN / PEN;
     const int grp = blockIdx.x % ngroups, b = blockIdx.x / ngroups;
     const size_t pencil = (size_t)grp * PEN + pen;   // sy * 2N + sx
-    double2 *p0 = W2 + ((size_t)(b0 + b) * N + j) * ZS + pencil;
+    double2 *p0 = W2 + ((size_t)(b0 + b) * nd + j) * ZS + pencil;
     const double *kh = Kt + pencil * RSK;
     double2 *bufA = smem + pen * Lay::PS, *bufB = bufA + PEN * Lay::PS;
     const TwGlobal twg{tw, j};
 
     double2 a[16], e[16];
 #pragma unroll
-    for (int r = 0; r < 16; ++r) a[r] = p0[(size_t)(T * r) * ZS];
+    for (int r = 0; r < 16; ++r) a[r] = (j + T * r < nd) ? p0[(size_t)(T * r) * ZS] : make_double2(0.0, 0.0);
     {
         double2 v[16];
         fwd_half<T, 0, Lay>(a, v, j, bufA, twg, SyncBlock());
@@ -414,7 +422,8 @@ k_z_conv_batch(const double *__restrict__ Kt, double2 *__restrict__ W2, const do
         inv_half<T, 1, Lay, false, true>(v, e, j, bufB, twg, SyncBlock(), kh + N);    // * K-hat, odd slots; e += odd half
     }
 #pragma unroll
-    for (int r = 0; r < 16; ++r) p0[(size_t)(T * r) * ZS] = e[r];
+    for (int r = 0; r < 16; ++r)
+        if (j + T * r < nd) p0[(size_t)(T * r) * ZS] = e[r];
 }
 
 }  // namespace cmk

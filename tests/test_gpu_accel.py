@@ -37,7 +37,7 @@ def _assert_parity(got, ref):
         assert e <= TOL * scale, f"level {l}: {e:.3e} > {TOL} * {scale:.3e}"
 
 
-@pytest.mark.parametrize("N,L", [(16, 1), (16, 2), (32, 3), (64, 4)])
+@pytest.mark.parametrize("N,L", [(16, 1), (16, 2), (32, 3), (64, 4), (20, 3), (48, 2), (96, 2), (168, 2)])
 def test_random_potentials(N, L):
     rng = np.random.default_rng(100 + N + L)
     phi = rng.standard_normal((L, N, N, N))

@@ -299,7 +299,7 @@ def test_G_scales_linearly_and_error_codes():
     assert np.abs(b - 6.674e-8 * a).max() <= 1e-15 * np.abs(b).max()
     p1.close()
     p2.close()
-    for bad in [dict(N=24, levels=2, dx0=1.0), dict(N=8, levels=2, dx0=1.0), dict(N=1024, levels=2, dx0=1.0),
+    for bad in [dict(N=26, levels=2, dx0=1.0), dict(N=8, levels=2, dx0=1.0), dict(N=516, levels=2, dx0=1.0),
                 dict(N=16, levels=0, dx0=1.0), dict(N=16, levels=2, dx0=0.0), dict(N=16, levels=2, dx0=1.0, refinement=3)]:
         with pytest.raises(pkg.CMError) as ei:
             pkg.cm_plan_create(**bad)
@@ -423,4 +423,44 @@ def test_results_do_not_depend_on_what_else_runs_on_the_gpu(N, L):
         plan.potential(rho, out)
         torch.cuda.synchronize()
         assert torch.equal(out, ref), f"repeat {rep}: result changed under co-scheduling"
+    plan.close()
+
+
+# ------------------------------------------------------------------ general sizes: any N % 4 == 0
+@pytest.mark.parametrize("N,L", [(20, 3), (24, 2), (28, 4), (36, 2), (48, 3)])
+def test_general_sizes_against_the_direct_sum_oracle(N, L):
+    """N % 4 == 0 is all the method needs (L76).  Sizes that are not powers of two run the same passes at the next power of
+    two (more zero padding): rows, planes, cavity geometry and the caller's arrays follow N.  Whole grids
+    against the brute-force O(N^6) oracle (its FFT path is radix-2 only), plus the host entry point."""
+    rng = np.random.default_rng(1000 + N)
+    rho = rng.random((L, N, N, N)) * (4.0 ** np.arange(L))[:, None, None, None]
+    got, plan = _solve_gpu(rho, 2.0 / N, G=1.3)
+    ref = oracle.solve(rho, 2.0 / N, G=1.3, method="direct")
+    _assert_parity(got, ref)
+    host = plan.potential_host(torch.from_numpy(rho).pin_memory())
+    torch.cuda.synchronize()
+    assert np.array_equal(host.numpy(), got)
+    plan.close()
+
+
+@pytest.mark.parametrize("N,L", [(96, 3), (192, 2), (320, 2)])
+def test_general_sizes_sampled_direct_sums(N, L):
+    """Larger sizes with factors 3 and 5 (transforms at 128 / 256 / 512): sampled outputs of every level against direct sums
+    (faces, corners, cavity ring, interior), and the invariants that hold at any size (mirror symmetry, zero in -> zero out)."""
+    rng = np.random.default_rng(2000 + N)
+    rho = rng.random((L, N, N, N)) * (4.0 ** np.arange(L))[:, None, None, None]
+    got, plan = _solve_gpu(rho, 2.0 / N)
+    Q = N // 4
+    targets = []
+    for l in range(L):
+        targets += [(l, 0, 0, 0), (l, N - 1, N - 1, N - 1), (l, N - 1, 0, N // 2), (l, Q - 1, Q, 3 * Q), (l, Q, Q, Q),
+                    (l, 3 * Q - 1, 3 * Q, Q - 1), (l, N // 2, N // 2 - 1, N // 3), (l, 5, N - 7, 2 * Q + 3)]
+    pts = oracle.solve_points(rho, 2.0 / N, targets)
+    for t, r in zip(targets, pts):
+        assert abs(got[t] - r) <= TOL * np.abs(got[t[0]]).max(), (t, got[t], r)
+    # mirror symmetry: flipping every level along x flips the result
+    d = torch.from_numpy(np.ascontiguousarray(rho[:, :, :, ::-1])).cuda()
+    flipped = plan.potential(d).cpu().numpy()[:, :, :, ::-1]
+    for l in range(L):
+        assert np.abs(flipped[l] - got[l]).max() <= TOL * np.abs(got[l]).max()
     plan.close()

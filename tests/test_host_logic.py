@@ -30,7 +30,7 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
 
 def test_argument_validation_needs_no_gpu():
     import paper_2301_06763_b200 as pkg
-    for kw in [dict(N=24, levels=2, dx0=1.0), dict(N=16, levels=2, dx0=-1.0), dict(N=16, levels=2, dx0=1.0, refinement=4)]:
+    for kw in [dict(N=26, levels=2, dx0=1.0), dict(N=12, levels=2, dx0=1.0), dict(N=520, levels=2, dx0=1.0), dict(N=16, levels=2, dx0=-1.0), dict(N=16, levels=2, dx0=1.0, refinement=4)]:
         with pytest.raises(pkg.CMError) as ei:
             pkg.cm_plan_create(**kw)
         assert ei.value.code == pkg.CM_EINVAL
