@@ -463,4 +463,7 @@ def test_general_sizes_sampled_direct_sums(N, L):
     flipped = plan.potential(d).cpu().numpy()[:, :, :, ::-1]
     for l in range(L):
         assert np.abs(flipped[l] - got[l]).max() <= TOL * np.abs(got[l]).max()
+    host = plan.potential_host(torch.from_numpy(rho).pin_memory())      # N >= 128: the level pipeline with the GEN kernels
+    torch.cuda.synchronize()
+    assert np.array_equal(host.numpy(), got)
     plan.close()
