@@ -133,10 +133,12 @@ __host__ __device__ __forceinline__ constexpr int freq_to_slot(int k, int N)   /
     return (k & 1) * N + 16 * (k >> 5) + ((k >> 1) & 15);
 }
 
+// DEC = 1 is the plain P3 of N = 512 plans (cm_lib.cu: no decimation, no E, every row read): levels b0 .. b0 + L - 1 of W2
+// (nd planes each) share the CTA's K-hat tile like the two mirror tiles do.
 template <int T, int DEC>
 __global__ void __launch_bounds__(batch_threads<T>(), 1)
 k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const double2 *__restrict__ tw,
-             const double2 *__restrict__ E, int zlo, int zhi)
+             const double2 *__restrict__ E, int zlo, int zhi, int b0, int L, int nd)
 {
     using C = ZDecCfg<T>;
     constexpr int N = C::N, NN = C::NN, PEN = C::PEN, GX = NN / PEN;   // GX pencil groups per sy row
@@ -169,15 +171,16 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
     }
     // twiddles and E feed multiplies directly: from global memory their latency was 26 % of the warp time (ncu, T = 32)
     for (int i = tid; i < 32 * T; i += batch_threads<T>()) tw_s[i] = __ldg(&tw[(i % T) * (i / T)]);
-    for (int i = tid; i < NN; i += batch_threads<T>()) E_s[i] = __ldg(&E[i]);
+    if (DEC > 1)
+        for (int i = tid; i < NN; i += batch_threads<T>()) E_s[i] = __ldg(&E[i]);
     __syncthreads();     // tables in place; the barrier is initialised before anyone waits on it
     const double *kh_s = reinterpret_cast<const double *>(smem_raw + C::OFF_KH) + pen * C::RSKH;
     const KhHalf<N> kh0{kh_s, 0}, kh1{kh_s + C::KE, 1};
     double2 *bufA = smem + pen * Lay::PS, *bufB = bufA + PEN * Lay::PS;
     const TwAllShared<T> twg{tw_s + j};
 
-    for (int t = 0; t < ntile; ++t) {
-        double2 *col = W2 + ((size_t)(t ? sy_b : sy_a) * NN + (size_t)gx * PEN + pen);
+    for (int t = 0; t < ntile * L; ++t) {
+        double2 *col = W2 + (size_t)(b0 + t / ntile) * nd * ZS + ((size_t)((t % ntile) ? sy_b : sy_a) * NN + (size_t)gx * PEN + pen);
         double2 a[16], e[16];
 #pragma unroll
         for (int r = 0; r < 16; ++r) {
@@ -187,14 +190,14 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
         {
             double2 v[16];
             fwd_half<T, 0, Lay>(a, v, j, bufA, twg, SyncBlock());
-            mul_E<T>(v, E_s, j);
+            if (DEC > 1) mul_E<T>(v, E_s, j);
             if (t == 0) mbar_wait(bar_k, 0);
             inv_half<T, 0, Lay, false, true, DEC>(v, e, j, bufB, twg, SyncBlock(), kh0);
         }
         {
             double2 v[16];
             fwd_half<T, 1, Lay>(a, v, j, bufA, twg, SyncBlock());
-            mul_E<T>(v, E_s + N, j);
+            if (DEC > 1) mul_E<T>(v, E_s + N, j);
             inv_half<T, 1, Lay, false, true, DEC>(v, e, j, bufB, twg, SyncBlock(), kh1);
         }
         if ((j % DEC) == 0) {

@@ -91,7 +91,7 @@ template <int T> int set_attrs(cm_plan *p)
         if constexpr (T >= 8)
             CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_warp<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZWarpCfg<T>::SMEM));
     } else {
-        CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_batch<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute(k_z_conv_dec<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZDecCfg<T>::SMEM));
     }
     return CM_OK;
 }
@@ -113,8 +113,10 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
         }
         k_z_conv_tma<T><<<grid, kThreads, ZConvCfg<T>::SMEM, s>>>(p->mapW, p->Khat, p->W2, p->tw, L, ngroups, b0, p->N);
     } else {
-        const unsigned ngroups = (unsigned)(NN * NN / batch_pencils<T>());
-        k_z_conv_batch<T><<<ngroups * (unsigned)L, batch_threads<T>(), smem_batch<T>(), s>>>(p->Khat, p->W2, p->tw, b0, p->N);
+        // N = 512: the batch-fastest P3 of cm_expand.cuh without decimation (a CTA per (|f_y|, 8 pencils): K-hat tile shared
+        // by the two mirror tiles and by the levels)
+        k_z_conv_dec<T, 1><<<(unsigned)((size_t)(N + 1) * (NN / batch_pencils<T>())), batch_threads<T>(), ZDecCfg<T>::SMEM, s>>>(
+            p->Khat, p->W2, p->tw, nullptr, 0, p->N, b0, L, p->N);
     }
 }
 
@@ -436,7 +438,7 @@ int cm_plan_create(cm_plan **out, int N, int levels, double dx0, int refinement)
         if (cuda_fail(p, cudaGetDevice(&dev), "cudaGetDevice") ||
             cuda_fail(p, cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
             rc = CM_ECUDA;
-        else if (p->Nf <= 256) rc = make_tensor_maps(p);   // the TMA-fed P3 (Nf = 512 runs k_z_conv_batch)
+        else if (p->Nf <= 256) rc = make_tensor_maps(p);   // the TMA-fed P3 (Nf = 512 runs k_z_conv_dec<32, 1>)
     }
     if (rc == CM_OK) {
         switch (p->T) {
@@ -602,7 +604,7 @@ template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, c
     const unsigned gr = (unsigned)(((size_t)Nc * Nc + ROWS - 1) / ROWS);
     k_x_fwd_blk<T><<<gr, kThreads, smem_row<T>(), s>>>(src_re, src_im, pe->W1, pe->tw, Nc, c0);
     k_y_fwd_blk<T><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W1, pe->W2, pe->tw, Nc, c0);
-    k_z_conv_dec<T, F><<<(unsigned)((size_t)(N + 1) * (NN / PEN)), BT, ZDecCfg<T>::SMEM, s>>>(pe->Khat, pe->W2, pe->tw, pe->decE, c0, c0 + Nc);
+    k_z_conv_dec<T, F><<<(unsigned)((size_t)(N + 1) * (NN / PEN)), BT, ZDecCfg<T>::SMEM, s>>>(pe->Khat, pe->W2, pe->tw, pe->decE, c0, c0 + Nc, 0, 1, 0);
     k_y_inv_dec<T, F><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W2, pe->W1, pe->tw, pe->decE, Nc);
     k_x_inv_dec<T, F><<<gr, kThreads, smem_row<T>(), s>>>(pe->W1, out_re, out_im, pe->tw, pe->decE, -1.0, Nc);
     CM_CUDA(pe, cudaGetLastError());

@@ -77,7 +77,7 @@ __device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.b
 __device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 
 template <int T> struct ZConvCfg {
-    static_assert(T <= 16, "the TMA-fed kernels cover N <= 256 (k_z_conv_batch above that)");
+    static_assert(T <= 16, "the TMA-fed kernels cover N <= 256 (k_z_conv_dec<32, 1> above that)");
     static constexpr int N = 16 * T, NN = 2 * N;
     static constexpr int PEN = kThreads / T;          // pencils per tile
     static constexpr int NBOX = PEN / 8;              // 128-byte column groups per tile
@@ -381,49 +381,6 @@ k_z_conv_warp(const __grid_constant__ CUtensorMap mapWw, const double *__restric
         }
     }
     if (lane == 0) tma_store_wait_all();
-}
-
-// ====================== P3 for N = 512 (T = 32): batch-fastest, straight from global memory =================
-// The TMA-fed kernels need the T threads of a pencil in one warp and a whole tile per 128-thread CTA; at T = 32 the
-// 32-point stage is split between the two half-warps of a pencil (divergent) and a tile would be 64 KB per stage.
-// N = 512 plans exist for the expanded grids of the modified method (single-level plans: no K-hat reuse across
-// levels), so this path is the plain one: the mapping of P2/P4 (lane = 8 adjacent pencils x 4 values of j, 256
-// threads per 8 pencils, the two halves of the 32-point stage in different warps), loads and stores straight
-// from/to registers in whole 128-byte lines, K-hat read from global memory, two exchange buffers used in turn.
-template <int T>
-__global__ void __launch_bounds__(batch_threads<T>(), 1)
-k_z_conv_batch(const double *__restrict__ Kt, double2 *__restrict__ W2, const double2 *__restrict__ tw, int b0, int nd)
-{
-    // nd <= N: z-rows of data per level (general sizes); rows beyond are zero on the way in and not written on the way out
-    constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>(), RSK = khat_row_stride(N);
-    constexpr size_t ZS = (size_t)NN * NN;           // stride of z in W2 (complex elements)
-    using Lay = LayBatch<T>;
-    extern __shared__ double2 smem[];
-    const int tid = threadIdx.x, px = tid & 7, j = (tid >> 3) % T, g = tid / (8 * T), pen = g * 8 + px;
-    const int ngroups = NN * NN / PEN;
-    const int grp = blockIdx.x % ngroups, b = blockIdx.x / ngroups;
-    const size_t pencil = (size_t)grp * PEN + pen;   // sy * 2N + sx
-    double2 *p0 = W2 + ((size_t)(b0 + b) * nd + j) * ZS + pencil;
-    const double *kh = Kt + pencil * RSK;
-    double2 *bufA = smem + pen * Lay::PS, *bufB = bufA + PEN * Lay::PS;
-    const TwGlobal twg{tw, j};
-
-    double2 a[16], e[16];
-#pragma unroll
-    for (int r = 0; r < 16; ++r) a[r] = (j + T * r < nd) ? p0[(size_t)(T * r) * ZS] : make_double2(0.0, 0.0);
-    {
-        double2 v[16];
-        fwd_half<T, 0, Lay>(a, v, j, bufA, twg, SyncBlock());
-        inv_half<T, 0, Lay, false, true>(v, e, j, bufB, twg, SyncBlock(), kh);        // * K-hat, even slots
-    }
-    {
-        double2 v[16];
-        fwd_half<T, 1, Lay>(a, v, j, bufA, twg, SyncBlock());
-        inv_half<T, 1, Lay, false, true>(v, e, j, bufB, twg, SyncBlock(), kh + N);    // * K-hat, odd slots; e += odd half
-    }
-#pragma unroll
-    for (int r = 0; r < 16; ++r)
-        if (j + T * r < nd) p0[(size_t)(T * r) * ZS] = e[r];
 }
 
 }  // namespace cmk
