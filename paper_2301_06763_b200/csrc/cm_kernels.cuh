@@ -72,15 +72,19 @@ struct TwGlobal {
     static constexpr bool RECUR = false;
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return __ldg(&tw[j * (2 * k1 + P)]); }
 };
-// P3 is bound by the shared-memory data pipe as much as by fp64 (profiles/): only every fourth twiddle (k1 = 0, 4, 8,
-// 12) is read from the table.  The ones between follow from the three-term recurrence of a geometric sequence,
+// P3 is bound by the shared-memory data pipe as much as by fp64 (profiles/): only every ANCH-th twiddle (k1 = 0, ANCH, ...)
+// is read from the table.  The ones between follow from the three-term recurrence of a geometric sequence,
 //     t[k+1] = 2 cos(phi) t[k] - t[k-1],   phi = arg of the ratio rho = w_2N^{2 j},
-// one FMA per component (a complex multiply by rho would be four); an anchor from the table every fourth step keeps
-// the rounding error at a few ulp (the recurrence amplifies it quadratically in the step count only).
-template <int T> struct TwShared {
+// one FMA per component (a complex multiply by rho would be four).  Its rounding error is ~1e-14 of a twiddle whatever the
+// anchor spacing (it is set by the cancellation in 2 cos(phi) at small phi, not by the step count: 1.1e-14 / 1.6e-14 /
+// 1.0e-14 at ANCH = 4 / 8 / 16), three orders below the parity bar.  ANCH is chosen per kernel by measurement
+// (profiles/r02_p3_experiments.md): 16 in the CTA-wide TMA kernel (one table read per exchange), 8 in the warp-autonomous
+// one (16 spills registers there).
+template <int T, int ANCH_ = 16> struct TwShared {
     const double2 *base;   // table + j
     double2 rho;           // w_2N^{2 j}
     static constexpr bool RECUR = true;
+    static constexpr int ANCH = ANCH_;
     template <int P> __device__ __forceinline__ double2 get(int k1) const { return base[(2 * k1 + P) * T]; }
 };
 
@@ -90,7 +94,7 @@ template <int P, class Tw> __device__ __forceinline__ double2 tw_next(const Tw &
 {
     double2 t;
     if constexpr (Tw::RECUR) {
-        if ((k1 & 3) == 0) t = (P == 0 && k1 == 0) ? make_double2(1.0, 0.0) : tw.template get<P>(k1);
+        if ((k1 & (Tw::ANCH - 1)) == 0) t = (P == 0 && k1 == 0) ? make_double2(1.0, 0.0) : tw.template get<P>(k1);
         else if (k1 == 1) t = (P == 0) ? tw.rho : cmul(c.p1, tw.rho);
         else {
             const double c2 = 2.0 * tw.rho.x;

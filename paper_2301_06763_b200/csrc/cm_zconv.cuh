@@ -280,13 +280,15 @@ k_z_conv_warp(const __grid_constant__ CUtensorMap mapWw, const double *__restric
     double2 *tw_s = reinterpret_cast<double2 *>(sbase + W::OFF_TW);
     const int pen = w * PPW + pxl;
 
-    if ((int)blockIdx.x >= ngroups) return;
-    const int my_groups = (ngroups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
-    const int ntiles = my_groups * L;
+    // the flat (group, level) tile list cut into equal ranges (balance: 4096 groups over 296 CTAs would leave 14 against
+    // 13.8 groups per CTA; -0.5 % at 8 x 128^3)
+    const long long total = (long long)ngroups * L;
+    const int t0 = (int)(total * blockIdx.x / gridDim.x);
+    const int ntiles = (int)(total * (blockIdx.x + 1) / gridDim.x) - t0;
+    if (ntiles <= 0) return;
     auto tile_of = [&](int t, int &g, int &b) {
-        const int gi = t / L;
-        b = t - gi * L;
-        g = (int)blockIdx.x + gi * (int)gridDim.x;
+        g = (t0 + t) / L;
+        b = (t0 + t) - g * L;
     };
     const uint32_t in_u = s0 + W::OFF_IN + w * WIN, ex_u = s0 + W::OFF_EX + w * EXW;
     unsigned char *in_p = sbase + W::OFF_IN + w * WIN, *out_p = sbase + W::OFF_EX + w * EXW;
@@ -318,7 +320,7 @@ k_z_conv_warp(const __grid_constant__ CUtensorMap mapWw, const double *__restric
         if (lane == 0) issue_in(g0, bb0);
     }
     const double *kh_p = reinterpret_cast<const double *>(sbase + W::OFF_KH) + pen * C::RSK;
-    const TwShared<T> tws{tw_s + j, tw_s[2 * T + j]};
+    const TwShared<T, 8> tws{tw_s + j, tw_s[2 * T + j]};
     // swizzled position of (row z, pencil pxl) in a warp's box: 32B rows: chunk bit0 ^= bit 7 of the offset;
     // 64B rows: chunk bits [1:0] ^= bits [8:7]
     auto box_off = [&](int z) -> uint32_t {
