@@ -177,6 +177,33 @@ int cm_plan_prepare_modified(cm_plan *plan, int depth, int qdp_direct);
  */
 int cm_direct_sum(cm_plan *plan, const double *rho_levels, int src_level, int dst_level, double *phi_dst, void *stream);
 
+/*
+ * cm_direct_sum for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same Eq. B.7 sum without a plan.  cm_direct_sum keeps its
+ * per-chunk partial sums in the plan's workspace; here they live in a file-scope __device__ array of
+ * CM_STATIC_SCRATCH_BYTES (4 MiB) that every GPU loading libcm holds until the process exits, so the call launches two
+ * kernels and calls no cudaMalloc, cudaFree or allocating library routine.
+ *   N               : cells per axis of both grids, 1 <= N <= CM_STATIC_MAX_N (the paper uses Eq. B.7 up to N = 32, L461);
+ *                     larger N is rejected with CM_EINVAL and cm_static_last_error() says why.
+ *   dx_src, dx_dst  : cell sizes of the source (finer) and target (coarser) grid, > 0; both grids are centred on the
+ *                     origin (cell i at (i + 1/2 - N/2) dx), as nested levels are.
+ *   G               : gravitational constant.
+ *   rho_src         : device, const, [N][N][N] fp64, x fastest: density of the source grid, read as given.
+ *   phi_dst         : device, [N][N][N] fp64, overwritten with Phi_ds on every cell of the target grid.
+ *   stream          : a cudaStream_t; the call enqueues and returns.
+ * The scratch array's device address is looked up once per device (cudaGetSymbolAddress, device current) — on the
+ * first call, or ahead of time by cm_direct_sum_static_setup() with that device current (do that before a capture).
+ * Every call on a device shares the array: it needs no clearing (a call writes every entry it later reads), but two
+ * calls that overlap on the GPU (two streams, graphs replayed side by side) race on it — serialise them.
+ * CM_EINVAL (size, NULL pointer, dx <= 0) or CM_ECUDA; the text is in cm_static_last_error() (thread-local, "" after
+ * a call that succeeded).
+ */
+#define CM_STATIC_MAX_N 32
+#define CM_STATIC_SCRATCH_BYTES (16u * 32u * 32u * 32u * 8u)
+int cm_direct_sum_static(int N, double dx_src, double dx_dst, double G, const double *rho_src, double *phi_dst, void *stream);
+int cm_direct_sum_static_setup(void);
+const char *cm_static_last_error(void);
+
 /* Release the plan and everything it owns.  NULL is accepted. */
 int cm_plan_destroy(cm_plan *plan);
 

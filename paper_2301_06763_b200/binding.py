@@ -20,7 +20,9 @@ EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potentia
            "cm_acceleration", "cm_potential_modified", "cm_potential_modified_triplets", "cm_plan_prepare_modified", "cm_direct_sum",
            "cm_plan_destroy",
            "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
-           "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error"]
+           "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error",
+           "cm_direct_sum_static", "cm_direct_sum_static_setup", "cm_static_last_error"]
+CM_STATIC_MAX_N = 32
 
 
 class CMError(RuntimeError):
@@ -57,6 +59,10 @@ def lib() -> C.CDLL:
     L.cm_error_string.restype = C.c_char_p
     L.cm_last_cuda_error.argtypes = [vp]
     L.cm_last_cuda_error.restype = C.c_char_p
+    L.cm_direct_sum_static.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, vp, vp, vp]
+    L.cm_direct_sum_static_setup.argtypes = []
+    L.cm_static_last_error.argtypes = []
+    L.cm_static_last_error.restype = C.c_char_p
     return L
 
 
@@ -111,6 +117,23 @@ def cm_direct_sum(plan: int, rho_ptr: int, src_level: int, dst_level: int, phi_p
     _check(lib().cm_direct_sum(plan, rho_ptr, int(src_level), int(dst_level), phi_ptr, stream), plan)
 
 
+def _check_static(code: int):
+    if code != CM_OK:
+        raise CMError(code, lib().cm_error_string(code).decode() + " (" + lib().cm_static_last_error().decode() + ")")
+
+
+def cm_direct_sum_static(N: int, dx_src: float, dx_dst: float, G: float, rho_ptr: int, phi_ptr: int, stream: int = 0) -> None:
+    _check_static(lib().cm_direct_sum_static(int(N), float(dx_src), float(dx_dst), float(G), rho_ptr, phi_ptr, stream))
+
+
+def cm_direct_sum_static_setup() -> None:
+    _check_static(lib().cm_direct_sum_static_setup())
+
+
+def cm_static_last_error() -> str:
+    return lib().cm_static_last_error().decode()
+
+
 def cm_acceleration(plan: int, phi_ptr: int, g_ptr: int, stream: int = 0) -> None:
     _check(lib().cm_acceleration(plan, phi_ptr, g_ptr, stream), plan)
 
@@ -139,7 +162,21 @@ def cm_slot_to_freq(N: int, slot: int) -> int:
     return int(lib().cm_slot_to_freq(N, slot))
 
 
-# ---- convenience wrapper over torch tensors (still marshalling only) ---------------
+# ---- convenience wrappers over torch tensors (still marshalling only) --------------
+def direct_sum_static(rho_src, dx_src: float, dx_dst: float, out, G: float = 1.0, stream=None):
+    """Eq. B.7 without a plan and without any allocation (cm_direct_sum_static): rho_src and out are CUDA float64
+    tensors [N, N, N] the caller owns, N <= CM_STATIC_MAX_N; out is overwritten and returned."""
+    import torch
+    N = int(rho_src.shape[0])
+    for t in (rho_src, out):
+        if t.dtype != torch.float64 or tuple(t.shape) != (N, N, N) or not t.is_contiguous() or t.device.type != "cuda":
+            raise ValueError(f"expected contiguous float64 cuda tensors of shape {(N, N, N)}")
+    s = torch.cuda.current_stream(rho_src.device).cuda_stream if stream is None else int(stream)
+    with torch.cuda.device(rho_src.device):
+        cm_direct_sum_static(N, dx_src, dx_dst, G, rho_src.data_ptr(), out.data_ptr(), s)
+    return out
+
+
 class Plan:
     """Owns a cm_plan; `potential` takes/returns CUDA float64 tensors [levels, N, N, N]."""
 
