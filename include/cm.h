@@ -97,6 +97,34 @@ int cm_potential(cm_plan *plan, const double *rho_levels, double *phi_levels, vo
 int cm_potential_host(cm_plan *plan, const double *rho_host, double *phi_host, void *stream);
 
 /*
+ * The solve sharded by levels across GPUs ("each of the three steps is independent and
+ * can be done in parallel"): one process per GPU, each with a plan of the WHOLE nest (same N, levels, dx0) and the
+ * densities / potentials of its own contiguous levels [lo, hi) only.  A solve is three calls with two small exchanges
+ * that the caller carries between neighbours (NCCL send/recv in paper_2301_06763_b200/sharded.py):
+ *
+ *   1. cm_shard_restrict  fine -> coarse: a1 on the own levels.  rc_from_finer (device, (N/2)^3 fp64; required iff
+ *      hi < levels, else NULL) is the density of level hi projected onto the cavity of level hi-1, received from the
+ *      owner of level hi; rc_to_coarser (device, (N/2)^3; iff lo > 0) receives the projection of level lo, to be sent
+ *      to the owner of level lo-1.
+ *   2. cm_shard_forward   P1..P4 (a2-a6) on the own levels; no exchange.
+ *   3. cm_shard_finish    coarse -> fine: P5 + a8 on the own levels.  ring_from_coarser (device, (N/2+2)^3 fp64; iff
+ *      lo > 0) is ext + Phi_hole of level lo-1 on its cavity grown by one cell — the box [N/4-1, 3N/4+1)^3, x fastest —
+ *      received from the owner of level lo-1; ring_to_finer (device, (N/2+2)^3; iff hi < levels) receives that box of
+ *      level hi-1.  phi_own is complete when the call's work on `stream` is.
+ *
+ *   rho_own / phi_own : device, [hi-lo][N][N][N] fp64, 16-byte aligned: levels lo .. hi-1.
+ * Same kernels and the same arithmetic as cm_potential: with lo = 0, hi = levels the three calls are cm_potential, and
+ * any partition gives bit-identical potentials.  The calls enqueue on `stream` and return.  CM_EINVAL for an empty or
+ * out-of-range [lo, hi) or a buffer that is present when it must be NULL (or the reverse); CM_ENOTREADY before
+ * cm_green_precompute.  One solve in flight per plan.
+ */
+int cm_shard_restrict(cm_plan *plan, const double *rho_own, int lo, int hi, const double *rc_from_finer, double *rc_to_coarser,
+                      void *stream);
+int cm_shard_forward(cm_plan *plan, const double *rho_own, int lo, int hi, void *stream);
+int cm_shard_finish(cm_plan *plan, double *phi_own, int lo, int hi, const double *ring_from_coarser, double *ring_to_finer,
+                    void *stream);
+
+/*
  * Measurement aid: the same solve launched kernel by kernel (no graph) with CUDA
  * events recorded on `stream` between the stages; synchronises `stream` and writes
  * the stage durations in milliseconds to ms_host[0..6] (host):

@@ -21,7 +21,8 @@ EXPORTS = ["cm_plan_create", "cm_green_precompute", "cm_potential", "cm_potentia
            "cm_plan_destroy",
            "cm_plan_set_G", "cm_plan_workspace_bytes", "cm_plan_kernel_launches", "cm_debug_copy",
            "cm_slot_to_freq", "cm_error_string", "cm_last_cuda_error",
-           "cm_direct_sum_static", "cm_direct_sum_static_setup", "cm_static_last_error"]
+           "cm_direct_sum_static", "cm_direct_sum_static_setup", "cm_static_last_error",
+           "cm_shard_restrict", "cm_shard_forward", "cm_shard_finish"]
 CM_STATIC_MAX_N = 32
 
 
@@ -59,6 +60,9 @@ def lib() -> C.CDLL:
     L.cm_error_string.restype = C.c_char_p
     L.cm_last_cuda_error.argtypes = [vp]
     L.cm_last_cuda_error.restype = C.c_char_p
+    L.cm_shard_restrict.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
+    L.cm_shard_forward.argtypes = [vp, vp, C.c_int, C.c_int, vp]
+    L.cm_shard_finish.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
     L.cm_direct_sum_static.argtypes = [C.c_int, C.c_double, C.c_double, C.c_double, vp, vp, vp]
     L.cm_direct_sum_static_setup.argtypes = []
     L.cm_static_last_error.argtypes = []
@@ -115,6 +119,18 @@ def cm_plan_prepare_modified(plan: int, depth: int, qdp_direct: int = 0) -> None
 
 def cm_direct_sum(plan: int, rho_ptr: int, src_level: int, dst_level: int, phi_ptr: int, stream: int = 0) -> None:
     _check(lib().cm_direct_sum(plan, rho_ptr, int(src_level), int(dst_level), phi_ptr, stream), plan)
+
+
+def cm_shard_restrict(plan: int, rho_own_ptr: int, lo: int, hi: int, rc_from_finer_ptr, rc_to_coarser_ptr, stream: int = 0) -> None:
+    _check(lib().cm_shard_restrict(plan, rho_own_ptr, int(lo), int(hi), rc_from_finer_ptr, rc_to_coarser_ptr, stream), plan)
+
+
+def cm_shard_forward(plan: int, rho_own_ptr: int, lo: int, hi: int, stream: int = 0) -> None:
+    _check(lib().cm_shard_forward(plan, rho_own_ptr, int(lo), int(hi), stream), plan)
+
+
+def cm_shard_finish(plan: int, phi_own_ptr: int, lo: int, hi: int, ring_from_coarser_ptr, ring_to_finer_ptr, stream: int = 0) -> None:
+    _check(lib().cm_shard_finish(plan, phi_own_ptr, int(lo), int(hi), ring_from_coarser_ptr, ring_to_finer_ptr, stream), plan)
 
 
 def _check_static(code: int):

@@ -582,6 +582,20 @@ __global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_
     rc_out[idx] = 0.125 * s;
 }
 
+// Level sharding across GPUs: all that a8 of level b reads of level b-1 is H = ext + Phi_hole on the
+// cavity grown by one cell, the box [N/4 - 1, 3N/4 + 1)^3.  Pack it into (N/2 + 2)^3 contiguous doubles for the
+// exchange, or unpack a received box into the level's slot of the hole buffer.
+__global__ void k_ring_box(int N, double *__restrict__ level, double *__restrict__ box, int unpack)
+{
+    const int B = N / 2 + 2, Q1 = N / 4 - 1;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (size_t)B * B * B) return;
+    const int x = (int)(i % B), y = (int)((i / B) % B), z = (int)(i / ((size_t)B * B));
+    double *c = level + ((size_t)(Q1 + z) * N + (Q1 + y)) * N + (Q1 + x);
+    if (unpack) *c = box[i];
+    else box[i] = *c;
+}
+
 // ============================ a0: Green's function ================================
 // g on the rearranged doubled mesh (Fig. 4): index a -> offset a (a <= N) or a - 2N.
 __global__ void k_green_sample(double2 *__restrict__ Gm, int N, double I0)

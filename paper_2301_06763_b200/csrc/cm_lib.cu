@@ -232,6 +232,46 @@ void dispatch_level(cm_plan *p, const double *rho, double *phi, cudaStream_t s, 
     }
 }
 
+// Levels [lo, hi) on their own (the level-sharded solve): the same kernels on those levels' rows of
+// W1 / W2, one launch per pass for the whole range (P3 reads K-hat once for the range).
+template <int T> void range_p1_to_p4(cm_plan *p, const double *rho, cudaStream_t s, int lo, int hi)
+{
+    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
+    const int nd = p->N, nl = hi - lo;
+    const size_t lrows = (size_t)nd * nd;
+    double2 *w1 = p->W1 + (size_t)lo * lrows * NN, *w2 = p->W2 + (size_t)lo * nd * NN * NN;
+    const unsigned gx = (unsigned)((nl * lrows + ROWS - 1) / ROWS), gy = (unsigned)((size_t)nl * nd * NN / PEN);
+    if (p->gen) {
+        k_x_fwd<T, true><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)lo * lrows, nd, (size_t)hi * lrows);
+        k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw, nd);
+        launch_zconv<T>(p, s, lo, nl);
+        k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw, nd);
+    } else {
+        k_x_fwd<T, false><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)lo * lrows);
+        k_y_fwd<T, false><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw);
+        launch_zconv<T>(p, s, lo, nl);
+        k_y_inv<T, false><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw);
+    }
+}
+template <int T> void range_p5(cm_plan *p, double *phi, cudaStream_t s, int lo, int hi)
+{
+    constexpr int ROWS = kThreads / T;
+    const size_t lrows = (size_t)p->N * p->N;
+    for (int b = lo; b < hi; ++b)      // the first launch of the range is a normal one: it comes after the unpacked ring
+        launch_x_inv<T>(p, phi, s, b, (unsigned)((lrows + ROWS - 1) / ROWS), -p->G * p->dx0 * p->dx0, /*chained=*/b > lo, 0);
+}
+void dispatch_range(cm_plan *p, const double *rho, double *phi, cudaStream_t s, int lo, int hi, bool p5)
+{
+    switch (p->T) {
+        case 1: p5 ? range_p5<1>(p, phi, s, lo, hi) : range_p1_to_p4<1>(p, rho, s, lo, hi); break;
+        case 2: p5 ? range_p5<2>(p, phi, s, lo, hi) : range_p1_to_p4<2>(p, rho, s, lo, hi); break;
+        case 4: p5 ? range_p5<4>(p, phi, s, lo, hi) : range_p1_to_p4<4>(p, rho, s, lo, hi); break;
+        case 8: p5 ? range_p5<8>(p, phi, s, lo, hi) : range_p1_to_p4<8>(p, rho, s, lo, hi); break;
+        case 16: p5 ? range_p5<16>(p, phi, s, lo, hi) : range_p1_to_p4<16>(p, rho, s, lo, hi); break;
+        case 32: p5 ? range_p5<32>(p, phi, s, lo, hi) : range_p1_to_p4<32>(p, rho, s, lo, hi); break;
+    }
+}
+
 // ev (optional): 8 events; ev[0] start, ev[1] after a1, ev[2..6] after P1..P5, ev[7] after a8
 // hole_all: P5 keeps H = Phi_hole + ext on every cell, not only on the ring the next level reads (the modified method, Eq. B.1)
 int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cudaEvent_t *ev = nullptr, int hole_all = 0)
@@ -575,6 +615,69 @@ int cm_potential_host(cm_plan *p, const double *rho_host, double *phi_host, void
     CM_CUDA(p, cudaGetLastError());
     CM_CUDA(p, cudaStreamSynchronize(p->copy_stream));
     CM_CUDA(p, cudaStreamSynchronize(s));
+    return CM_OK;
+}
+
+}  // extern "C"
+
+// ---- level-sharded solve: levels [lo, hi) of the nest on this GPU ----
+namespace {
+int check_shard(const cm_plan *p, const void *own, int lo, int hi)
+{
+    if (!p || !own || ((uintptr_t)own & 15)) return CM_EINVAL;
+    if (lo < 0 || hi <= lo || hi > p->L) return CM_EINVAL;
+    if (!p->green_ready) return CM_ENOTREADY;
+    return CM_OK;
+}
+// the caller's arrays hold the levels [lo, hi) only: address of the (virtual) level 0
+template <class Tp> Tp *level0(Tp *own, int lo, size_t n3) { return (Tp *)((uintptr_t)own - (uintptr_t)lo * n3 * sizeof(double)); }
+}  // namespace
+
+extern "C" {
+
+int cm_shard_restrict(cm_plan *p, const double *rho_own, int lo, int hi, const double *rc_from_finer, double *rc_to_coarser, void *stream)
+{
+    const int chk = check_shard(p, rho_own, lo, hi);
+    if (chk != CM_OK) return chk;
+    const int L = p->L;
+    if ((hi < L) != (rc_from_finer != nullptr) || (lo > 0) != (rc_to_coarser != nullptr)) return CM_EINVAL;
+    const size_t n3 = (size_t)p->N * p->N * p->N, h3 = n3 / 8;
+    const double *rho = level0(rho_own, lo, n3);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (hi < L) CM_CUDA(p, cudaMemcpyAsync(p->rc + h3 * (hi - 1), rc_from_finer, h3 * sizeof(double), cudaMemcpyDeviceToDevice, s));
+    // a1 on the own levels, fine -> coarse: level lf projects onto the cavity of level lf - 1; the last one leaves
+    for (int lf = hi - 1; lf >= lo && lf >= 1; --lf) {
+        const double *rc_f = (lf < L - 1) ? p->rc + h3 * lf : nullptr;
+        double *out = (lf - 1 >= lo) ? p->rc + h3 * (lf - 1) : rc_to_coarser;
+        k_restrict<<<(unsigned)((h3 + 255) / 256), 256, 0, s>>>(p->N, lf, L, rho + n3 * lf, rc_f, out);
+    }
+    CM_CUDA(p, cudaGetLastError());
+    return CM_OK;
+}
+
+int cm_shard_forward(cm_plan *p, const double *rho_own, int lo, int hi, void *stream)
+{
+    const int chk = check_shard(p, rho_own, lo, hi);
+    if (chk != CM_OK) return chk;
+    const size_t n3 = (size_t)p->N * p->N * p->N;
+    dispatch_range(p, level0(rho_own, lo, n3), nullptr, (cudaStream_t)stream, lo, hi, false);
+    CM_CUDA(p, cudaGetLastError());
+    return CM_OK;
+}
+
+int cm_shard_finish(cm_plan *p, double *phi_own, int lo, int hi, const double *ring_from_coarser, double *ring_to_finer, void *stream)
+{
+    const int chk = check_shard(p, phi_own, lo, hi);
+    if (chk != CM_OK) return chk;
+    const int L = p->L, B = p->N / 2 + 2;
+    if ((lo > 0) != (ring_from_coarser != nullptr) || (hi < L) != (ring_to_finer != nullptr)) return CM_EINVAL;
+    const size_t n3 = (size_t)p->N * p->N * p->N, b3 = (size_t)B * B * B;
+    const unsigned gb = (unsigned)((b3 + 255) / 256);
+    cudaStream_t s = (cudaStream_t)stream;
+    if (lo > 0) k_ring_box<<<gb, 256, 0, s>>>(p->N, p->hole + n3 * (lo - 1), const_cast<double *>(ring_from_coarser), 1);
+    dispatch_range(p, nullptr, level0(phi_own, lo, n3), s, lo, hi, true);
+    if (hi < L) k_ring_box<<<gb, 256, 0, s>>>(p->N, p->hole + n3 * (hi - 1), ring_to_finer, 0);
+    CM_CUDA(p, cudaGetLastError());
     return CM_OK;
 }
 
