@@ -630,6 +630,78 @@ def run_ours(args) -> None:
         dist.destroy_process_group()
 
 
+def run_sharded(args) -> None:
+    """`--shard-levels`: ONE solve of the config spread over the N ranks by levels (paper_2301_06763_b200/sharded.py,
+    SURVEY.md §8e) — strong scaling, against the default mode's replicas.  Each rank holds and solves its own levels;
+    the two neighbour exchanges (NCCL send/recv) are inside the timed region.  With N = 1 it times the three shard
+    calls (no CUDA graph) against cm_potential.  Untested on more than one GPU in this repository's runs."""
+    import torch
+    import workloads
+    import paper_2301_06763_b200 as pkg
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    else:                                            # a one-rank group so that the same code runs on one GPU
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        dist.init_process_group("gloo", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
+    cfg = workloads.CONFIGS[args.config]
+    N, L = cfg["N"], cfg["L"]
+    solver = pkg.ShardedSolver(N, L, 2.0 / N)
+    lo, hi = solver.lo, solver.hi
+    rho_own = torch.from_numpy(workloads.make_rho(args.config)[lo:hi].copy()).to(dev)
+    phi_own = torch.empty_like(rho_own)
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        solver.solve(rho_own, phi_own)
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(args.steps):
+        solver.solve(rho_own, phi_own)
+    e1.record(stream)
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1) / args.steps], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item())
+    clocks = sampler.stop() if rank == 0 else {}
+    # kernels of this rank's solve: k_restrict per own level >= 1, P1..P4, one P5 per level, k_ring_box per neighbour
+    launches = 0 if hi == lo else max(0, hi - max(lo, 1)) + 4 + (hi - lo) + int(lo > 0) + int(hi < L)
+    if rank == 0:
+        H, B = N // 2, N // 2 + 2
+        print(json.dumps({
+            "metric": METRIC, "value": L * N ** 3 / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "solves_per_s": 1.0 / (ms_step * 1e-3),
+            "config": {"workload": f"config {args.config}: {cfg['name']}", "N": N, "levels": L, "fields": 2 * L - 1,
+                       "parallelism": f"one solve, levels over {world} rank(s): {pkg.partition_levels(L, world)}",
+                       "exchange_bytes_per_boundary": {"fine_to_coarse": 8 * H ** 3, "coarse_to_fine": 8 * B ** 3},
+                       "l2": "inputs larger than L2" if N >= 128 else "not flushed (sharded mode is a scaling probe)",
+                       "launch": "cm_shard_restrict / cm_shard_forward / cm_shard_finish, kernel by kernel"},
+            "clocks": clocks, "e2e": None, "gpu_launches": args.steps * int(launches), "roofline": None, "cpu_baseline": None,
+        }), flush=True)
+    solver.close()
+    dist.destroy_process_group()
+
+
 def cufft_dense_reference(N: int, L: int, torch) -> dict:
     """Context only (--cufft-ref): the paper's own GPU scheme on this GPU — per field a dense
     zero-padded (2N)^3 cuFFT D2Z, a pointwise multiply and a Z2D, here through torch.fft; restriction,
@@ -669,10 +741,14 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the compact config-3 / config-4 lines")
     ap.add_argument("--cufft-ref", action="store_true", help="also time the paper's dense cuFFT scheme (context)")
+    ap.add_argument("--shard-levels", action="store_true",
+                    help="one solve spread over the ranks by levels (strong scaling) instead of one replica per rank")
     args = ap.parse_args()
     ensure_world(args.gpus, sys.argv[1:])
     if args.impl == "reference":
         run_reference(args)
+    elif args.shard_levels:
+        run_sharded(args)
     else:
         run_ours(args)
 
