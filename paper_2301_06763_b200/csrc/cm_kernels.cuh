@@ -559,7 +559,7 @@ __global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(c
 // ============================ a1: restriction cascade ==============================
 // rc[lf-1][ck][cj][ci] = mean of the 8 children of fine level lf, where a child that lies
 // under level lf+1 takes the already projected value rc[lf] (L280-L282; readings 9, 10).
-__global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_f, const double *__restrict__ rc_f,
+static __global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_f, const double *__restrict__ rc_f,
                            double *__restrict__ rc_out)
 {
     const int H = N / 2, Q = N / 4;
@@ -585,7 +585,7 @@ __global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_
 // Level sharding across GPUs: all that a8 of level b reads of level b-1 is H = ext + Phi_hole on the
 // cavity grown by one cell, the box [N/4 - 1, 3N/4 + 1)^3.  Pack it into (N/2 + 2)^3 contiguous doubles for the
 // exchange, or unpack a received box into the level's slot of the hole buffer.
-__global__ void k_ring_box(int N, double *__restrict__ level, double *__restrict__ box, int unpack)
+static __global__ void k_ring_box(int N, double *__restrict__ level, double *__restrict__ box, int unpack)
 {
     const int B = N / 2 + 2, Q1 = N / 4 - 1;
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -598,7 +598,7 @@ __global__ void k_ring_box(int N, double *__restrict__ level, double *__restrict
 
 // ============================ a0: Green's function ================================
 // g on the rearranged doubled mesh (Fig. 4): index a -> offset a (a <= N) or a - 2N.
-__global__ void k_green_sample(double2 *__restrict__ Gm, int N, double I0)
+static __global__ void k_green_sample(double2 *__restrict__ Gm, int N, double I0)
 {
     const int n = 2 * N;
     const size_t tot = (size_t)n * n * n;
@@ -612,7 +612,7 @@ __global__ void k_green_sample(double2 *__restrict__ Gm, int N, double I0)
 
 // Plain in-place radix-2 transform of one pencil per CTA (one-time set-up, not the hot
 // path): n = 2N points, n/2 threads, natural order in and out.
-__global__ void k_fft_simple(double2 *__restrict__ data, int n, int log2n, int axis, const double2 *__restrict__ tw)
+static __global__ void k_fft_simple(double2 *__restrict__ data, int n, int log2n, int axis, const double2 *__restrict__ tw)
 {
     extern __shared__ double2 sm[];
     const size_t u = blockIdx.x / n, v = blockIdx.x % n;
@@ -646,7 +646,7 @@ __host__ __device__ constexpr int khat_row_stride(int N) { return 2 * N + (N / 1
 
 // K-hat, pencil-major: Kt[(sy 2N + sx) RSK + sz] = Re Ghat[f(sz)][f(sy)][f(sx)] / (2N)^3, f = slot_to_freq.  The PEN
 // pencils of one P3 tile are one contiguous block, fetched by a single bulk copy and read as it lies.
-__global__ void k_green_permute(const double2 *__restrict__ Gm, double *__restrict__ Kt, int N)
+static __global__ void k_green_permute(const double2 *__restrict__ Gm, double *__restrict__ Kt, int N)
 {
     const int n = 2 * N, RSK = khat_row_stride(N);
     const size_t tot = (size_t)n * n * n;
@@ -658,7 +658,7 @@ __global__ void k_green_permute(const double2 *__restrict__ Gm, double *__restri
     }
 }
 // test access: the same values as [sz][sy][sx]
-__global__ void k_khat_export(const double *__restrict__ Kt, double *__restrict__ out, int N)
+static __global__ void k_khat_export(const double *__restrict__ Kt, double *__restrict__ out, int N)
 {
     const int n = 2 * N, RSK = khat_row_stride(N);
     const size_t tot = (size_t)n * n * n;
@@ -675,7 +675,7 @@ __global__ void k_khat_export(const double *__restrict__ Kt, double *__restrict_
 // and the outer boundary of level 0 uses the second-order one-sided difference.
 
 // pbar[l][ck][cj][ci] = mean of the 8 children (level l+1) of cavity cell (N/4 + c*) of level l.
-__global__ void k_child_mean(int N, int L, const double *__restrict__ phi, double *__restrict__ pbar)
+static __global__ void k_child_mean(int N, int L, const double *__restrict__ phi, double *__restrict__ pbar)
 {
     const int H = N / 2;
     const size_t h3 = (size_t)H * H * H, n3 = (size_t)N * N * N;
@@ -740,9 +740,9 @@ struct AccelField {
 // the general (face / cavity) case of one pair of cells, kept out of line so that the streaming
 // loop of k_accel stays small in registers
 // the one ghost value beyond an x face, out of line as well
-__device__ __noinline__ double accel_ghost_x(const AccelField F, int k, int j, int i) { return F.ghost(k, j, i, 0); }
+static __device__ __noinline__ double accel_ghost_x(const AccelField F, int k, int j, int i) { return F.ghost(k, j, i, 0); }
 
-__device__ __noinline__ void accel_pair_general(const AccelField F, int k, int j, int i, double inv, double2 &gx,
+static __device__ __noinline__ void accel_pair_general(const AccelField F, int k, int j, int i, double inv, double2 &gx,
                                                 double2 &gy, double2 &gz)
 {
     const double c0 = F.at(k, j, i, 0), c1 = F.at(k, j, i + 1, 0);
@@ -753,7 +753,7 @@ __device__ __noinline__ void accel_pair_general(const AccelField F, int k, int j
                       -(F.at(k + 1, j, i + 1, 2) - F.at(k - 1, j, i + 1, 2)) * inv);
 }
 
-__global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, int ZCH, double dx0, const double *__restrict__ phi,
+static __global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, int ZCH, double dx0, const double *__restrict__ phi,
                                                const double *__restrict__ pbar, double *__restrict__ g)
 {
     const size_t n3 = (size_t)N * N * N, h3 = n3 / 8, nn = (size_t)N * N;
@@ -807,7 +807,7 @@ __global__ void __launch_bounds__(256, 4) k_accel(int N, int L, int TX, int TY, 
 // rho-bar of level l1 as a compact N^3 array: the level's density with the finer levels projected onto it (rc);
 // `hole`: its own cavity zeroed (the doubled grid "with a central hole" of the triplet scheme, so that grid l1+1's
 // mass is not counted twice).  The expanded grid around it is never materialised (cm_expand.cuh).
-__global__ void k_level_density(int N, int hole, int l1, int L, const double *__restrict__ rho, const double *__restrict__ rc,
+static __global__ void k_level_density(int N, int hole, int l1, int L, const double *__restrict__ rho, const double *__restrict__ rc,
                                 double *__restrict__ out)
 {
     const int H = N / 2, Q = N / 4;
@@ -823,7 +823,7 @@ __global__ void k_level_density(int N, int hole, int l1, int L, const double *__
 }
 
 // phi_n = base + scale * add   (the "reduce" of B.1 / B.3: `add` holds the block sums the decimated passes formed)
-__global__ void k_add_scaled(size_t n, const double *base, const double *__restrict__ add, double scale, double *phi_n)
+static __global__ void k_add_scaled(size_t n, const double *base, const double *__restrict__ add, double scale, double *phi_n)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx < n) phi_n[idx] = base[idx] + scale * add[idx];
@@ -836,7 +836,7 @@ __global__ void k_add_scaled(size_t n, const double *base, const double *__restr
 // in tiles of 256.  fp64 ALU-bound: N^6 inverse square roots; the paper uses it for N <= 32 only.
 // gridDim.y source chunks (so that small grids still fill the GPU): chunk c sums sources [c, c+1) * n3 / gridDim.y
 // into part[c][t]; k_direct_reduce adds the chunks in a fixed order (deterministic).
-__global__ void __launch_bounds__(256) k_direct_sum(int N, double dxs, double dxd, const double *__restrict__ rho_src,
+static __global__ void __launch_bounds__(256) k_direct_sum(int N, double dxs, double dxd, const double *__restrict__ rho_src,
                                                     double *__restrict__ part)
 {
     __shared__ double4 src[256];
@@ -867,7 +867,7 @@ __global__ void __launch_bounds__(256) k_direct_sum(int N, double dxs, double dx
     }
     if (t < n3) part[(size_t)blockIdx.y * n3 + t] = acc;
 }
-__global__ void k_direct_reduce(size_t n3, int chunks, double G, const double *__restrict__ part, double *__restrict__ phi_dst)
+static __global__ void k_direct_reduce(size_t n3, int chunks, double G, const double *__restrict__ part, double *__restrict__ phi_dst)
 {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n3) return;

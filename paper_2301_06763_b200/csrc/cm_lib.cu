@@ -1,76 +1,12 @@
-// cm_lib.cu — the C ABI of include/cm.h: plan, workspace, CUDA-graph capture.
-#include <cuda_runtime.h>
-
-#include <cmath>
-#include <cstdio>
-#include <cstdlib>
-#include <cstring>
-#include <new>
-#include <vector>
-
-#include "../../include/cm.h"
-#include "cm_kernels.cuh"
+// cm_lib.cu — the C ABI of include/cm.h: plan, workspace, CUDA-graph capture (the expanded-grid passes of the modified
+// method are in cm_lib_expand.cu, the allocation-free direct sum in cm_static.cu).
+#include "cm_plan.h"
 #include "cm_zconv.cuh"
 #include "cm_expand.cuh"
 
 namespace {
 
-struct GraphEntry {
-    const double *rho;
-    double *phi;
-    int mode;                      // 0 cm_potential, 1 pairs, 2 triplets (quadrupled grid by FFT), 3 triplets (Eq. B.7)
-    cudaGraphExec_t exec;
-    unsigned long long last_use;   // for least-recently-used eviction
-};
-constexpr size_t kGraphCacheSize = 8;
-
-}  // namespace
-
-struct cm_plan {
-    int N = 0, L = 0, T = 0;       // N: cells per axis of a level; the transforms run at Nf = 16 T = the next power of two >= N
-    int Nf = 0;
-    bool gen = false;               // N < Nf: the general-size instantiations of the passes
-    double dx0 = 0, G = 1.0;
-    double2 *W1 = nullptr, *W2 = nullptr, *tw = nullptr;
-    double *Khat = nullptr, *rc = nullptr, *hole = nullptr, *pbar = nullptr;
-    double *stage_rho = nullptr, *stage_phi = nullptr;
-    size_t bytes = 0;
-    bool green_ready = false;
-    bool split_x = false, split_y = false;   // P1 / P2 split by output parity (256-thread CTAs): N = 256
-    cm_plan *dbl = nullptr, *qdp = nullptr;   // single-level plans of the doubled (2N)^3 and quadrupled (4N)^3 fine grid
-    double *rho4 = nullptr, *phi4 = nullptr, *tmp3 = nullptr;
-    double *rho2 = nullptr, *phi2 = nullptr;   // two doubled grids each: one complex solve serves two pairs
-    double2 *decE = nullptr;                    // expanded-grid plans: E(k) of the decimated inverse, slot order (cm_expand.cuh)
-    bool use_graph = true;
-    cudaStream_t cap_stream = nullptr, copy_stream = nullptr;
-    std::vector<cudaEvent_t> ev_level;   // cm_potential_host's pipeline: [0,32) level arrived, [32,64) level's Phi ready, [64] start
-    std::vector<GraphEntry> graphs;
-    unsigned long long use_counter = 0;
-    int launches = 0;
-    int num_sms = 148;
-    CUtensorMap mapW, mapWw;        // W2 as CTA-wide 128-byte boxes / as per-warp 32- or 64-byte boxes (k_z_conv_warp)
-    bool zconv_warp = false;
-    int kernels_per_solve = 0;
-    char err[512] = {0};
-};
-
-namespace {
-
 using namespace cmk;
-
-bool cuda_fail(cm_plan *p, cudaError_t e, const char *what)
-{
-    if (e == cudaSuccess) return false;
-    if (p) std::snprintf(p->err, sizeof(p->err), "%s: %s", what, cudaGetErrorString(e));
-    return true;
-}
-#define CM_CUDA(p, call)                                  \
-    do {                                                  \
-        if (cuda_fail((p), (call), #call)) return CM_ECUDA; \
-    } while (0)
-
-template <int T> size_t smem_row() { return sizeof(double2) * 2 * (kThreads / T) * LayRow<T>::PS; }
-template <int T> size_t smem_batch() { return sizeof(double2) * 2 * batch_pencils<T>() * LayBatch<T>::PS; }
 
 template <int T> int set_attrs(cm_plan *p)
 {
@@ -685,46 +621,6 @@ int cm_shard_finish(cm_plan *p, double *phi_own, int lo, int hi, const double *r
 
 namespace {
 
-// The five passes of an expanded-grid solve (cm_expand.cuh) on the single-level plan pe of size N' = 16 T = F Nc:
-// forward passes pruned to the central Nc^3 block, inverse passes decimated by F.  src_re / src_im: compact Nc^3
-// densities (src_im optional: the second real field); out_re / out_im: minus the block SUMS of their potentials.
-template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, const double *src_im, double *out_re, double *out_im,
-                                            cudaStream_t s, bool attrs_only)
-{
-    constexpr int N = 16 * T, NN = 2 * N, ROWS = kThreads / T, PEN = batch_pencils<T>(), BT = batch_threads<T>();
-    static bool attrs = false;      // per instantiation; the attribute is per function, not per plan
-    if (!attrs) {
-        CM_CUDA(pe, cudaFuncSetAttribute(k_x_fwd_blk<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
-        CM_CUDA(pe, cudaFuncSetAttribute(k_y_fwd_blk<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-        CM_CUDA(pe, cudaFuncSetAttribute(k_z_conv_dec<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ZDecCfg<T>::SMEM));
-        CM_CUDA(pe, cudaFuncSetAttribute(k_y_inv_dec<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
-        CM_CUDA(pe, cudaFuncSetAttribute(k_x_inv_dec<T, F>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
-        attrs = true;
-    }
-    if (attrs_only) return CM_OK;
-    // the expanded grid has pe->N = F Nc cells per axis (transformed at N = 16 T >= pe->N); the block sits in its middle
-    const int Nc = pe->N / F, c0 = (pe->N - Nc) / 2;
-    const unsigned gr = (unsigned)(((size_t)Nc * Nc + ROWS - 1) / ROWS);
-    k_x_fwd_blk<T><<<gr, kThreads, smem_row<T>(), s>>>(src_re, src_im, pe->W1, pe->tw, Nc, c0);
-    k_y_fwd_blk<T><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W1, pe->W2, pe->tw, Nc, c0);
-    k_z_conv_dec<T, F><<<(unsigned)((size_t)(N + 1) * (NN / PEN)), BT, ZDecCfg<T>::SMEM, s>>>(pe->Khat, pe->W2, pe->tw, pe->decE, c0, c0 + Nc, 0, 1, 0);
-    k_y_inv_dec<T, F><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W2, pe->W1, pe->tw, pe->decE, Nc);
-    k_x_inv_dec<T, F><<<gr, kThreads, smem_row<T>(), s>>>(pe->W1, out_re, out_im, pe->tw, pe->decE, -1.0, Nc);
-    CM_CUDA(pe, cudaGetLastError());
-    return CM_OK;
-}
-
-int dispatch_expanded(cm_plan *pe, int F, const double *src_re, const double *src_im, double *out_re, double *out_im, cudaStream_t s,
-                      bool attrs_only = false)
-{
-#define CM_EXP(TT, FF) \
-    if (pe->T == TT && F == FF) return expanded_passes<TT, FF>(pe, src_re, src_im, out_re, out_im, s, attrs_only);
-    CM_EXP(2, 2) CM_EXP(4, 2) CM_EXP(8, 2) CM_EXP(16, 2) CM_EXP(32, 2)
-    CM_EXP(4, 4) CM_EXP(8, 4) CM_EXP(16, 4) CM_EXP(32, 4)
-#undef CM_EXP
-    return CM_EINVAL;
-}
-
 // one expanded-grid plan (N' = F N, one level, unit G and dx: it supplies K-hat, the twiddles and W1 / W2), the table
 // E(k) = sum_{q<F} e^{2 pi i k q / 2N'} in slot order, and compact N^3 buffers for two sources and two results
 int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **src, double **res)
@@ -755,7 +651,7 @@ int ensure_expanded(cm_plan *p, int F, cm_plan **plan, double **src, double **re
             if (cuda_fail(p, cudaMemcpy(pe->decE, E.data(), n * sizeof(double2), cudaMemcpyHostToDevice), "cudaMemcpy(E)")) rc = CM_ECUDA;
         }
     }
-    if (rc == CM_OK) rc = dispatch_expanded(*plan, F, nullptr, nullptr, nullptr, nullptr, nullptr, /*attrs_only=*/true);
+    if (rc == CM_OK) rc = cm_dispatch_expanded(*plan, F, nullptr, nullptr, nullptr, nullptr, nullptr, /*attrs_only=*/true);
     if (rc == CM_OK && !*src) rc = dev_alloc(p, src, 2 * n3);
     if (rc == CM_OK && !*res) rc = dev_alloc(p, res, 2 * n3);
     if (rc != CM_OK) {
@@ -783,7 +679,7 @@ int solve_expanded(cm_plan *p, cm_plan *pe, int F, const double *rho, double *sr
     const unsigned g = (unsigned)((n3 + 255) / 256);
     k_level_density<<<g, 256, 0, s>>>(p->N, hole1, l1, p->L, rho, p->rc, src);          // rho-bar of grid l1 (optionally holed)
     if (l1b >= 0) k_level_density<<<g, 256, 0, s>>>(p->N, hole1b, l1b, p->L, rho, p->rc, src + n3);
-    return dispatch_expanded(pe, F, src, l1b >= 0 ? src + n3 : nullptr, res, l1b >= 0 ? res + n3 : nullptr, s);
+    return cm_dispatch_expanded(pe, F, src, l1b >= 0 ? src + n3 : nullptr, res, l1b >= 0 ? res + n3 : nullptr, s, /*attrs_only=*/false);
 }
 
 int direct_sum_impl(cm_plan *p, const double *rho_src, int src_level, int dst_level, double *phi_dst, cudaStream_t s);
