@@ -502,7 +502,7 @@ struct SyncParity {
 };
 template <int T>
 __global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *__restrict__ W1, double2 *__restrict__ W2,
-                                                                 const double2 *__restrict__ tw)
+                                                                 const double2 *__restrict__ tw, int ahead)
 {
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     using Lay = LayBatch<T>;
@@ -518,6 +518,18 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *
     double2 a[16], v[16];
 #pragma unroll
     for (int r = 0; r < 16; ++r) a[r] = src[(size_t)(j + T * r) * NN];
+    {   // Pull the input of the tile `ahead` CTAs later into L2 (one lane per 128-byte line).  ncu: 55 % of this kernel's
+        // stall samples sit on the load scoreboard and it moves 5.8 TB/s where P4 — the same bytes the other way round, twice
+        // the unique loads per CTA in flight — reaches the copy peak; registers (128 x 512 threads = the whole file) leave no
+        // room for a second tile.  With the next wave's columns already in L2 the load phase shrinks: 2.78 -> 2.59 ms at
+        // 10 x 256^3 (ahead = 148 = half a wave of CTAs; 74 ... 444 within 3 %; profiles/r02_pass_variants.md).
+        if (ahead > 0 && P == 0 && px == 0 && blockIdx.x + ahead < gridDim.x) {
+            const size_t q2 = (size_t)(blockIdx.x + ahead) * PEN + g * 8;
+            const double2 *s2 = W1 + (q2 / NN) * N * NN + (q2 % NN);
+#pragma unroll
+            for (int r = 0; r < 16; ++r) asm volatile("prefetch.global.L2 [%0];" ::"l"(s2 + (size_t)(j + T * r) * NN));
+        }
+    }
     if (P == 0) fwd_half<T, 0, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncParity{1});
     else fwd_half<T, 1, Lay>(a, v, j, buf, TwGlobal{tw, j}, SyncParity{2});
 #pragma unroll

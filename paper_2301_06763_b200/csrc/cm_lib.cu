@@ -105,7 +105,7 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     if (ev) cudaEventRecord(ev[2], s);
     if constexpr (T <= 16) {
         if (p->split_y) {
-            k_y_fwd_split<T><<<gy, 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
+            k_y_fwd_split<T><<<gy, 2 * kThreads, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, /*ahead=*/p->num_sms);
             done_y = true;
         }
     }
