@@ -571,14 +571,10 @@ __global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(c
 // ============================ a1: restriction cascade ==============================
 // rc[lf-1][ck][cj][ci] = mean of the 8 children of fine level lf, where a child that lies
 // under level lf+1 takes the already projected value rc[lf] (L280-L282; readings 9, 10).
-static __global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_f, const double *__restrict__ rc_f,
-                           double *__restrict__ rc_out)
+__device__ __forceinline__ double restrict_cell(int N, bool use_rc, const double *__restrict__ rho_f, const double *__restrict__ rc_f,
+                                                int ci, int cj, int ck)
 {
     const int H = N / 2, Q = N / 4;
-    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= H * H * H) return;
-    const int ci = idx % H, cj = (idx / H) % H, ck = idx / (H * H);
-    const bool use_rc = (lf < L - 1);
     double s = 0.0;
 #pragma unroll
     for (int c = 0; c < 2; ++c)
@@ -591,7 +587,51 @@ static __global__ void k_restrict(int N, int lf, int L, const double *__restrict
                 s += cav ? rc_f[((size_t)(k - Q) * H + (jx - Q)) * H + (i - Q)]
                          : rho_f[((size_t)k * N + jx) * N + i];
             }
-    rc_out[idx] = 0.125 * s;
+    return 0.125 * s;
+}
+static __global__ void k_restrict(int N, int lf, int L, const double *__restrict__ rho_f, const double *__restrict__ rc_f,
+                                  double *__restrict__ rc_out)
+{
+    const int H = N / 2;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= H * H * H) return;
+    rc_out[idx] = restrict_cell(N, lf < L - 1, rho_f, rc_f, idx % H, (idx / H) % H, idx / (H * H));
+}
+// The cascade is sequential only where a parent has a child under the next finer grid: the box [I0, I1)^3 of parents,
+// I0 = N/8 (rounded down), I1 = 3N/8 (rounded up) — 1/8 of a level's outputs.  cm_potential therefore runs a1 as ONE launch
+// over every level for the parents outside that box (all parents of the finest level), which read rho only, and then
+// fine -> coarse one small launch per level for the box.  Same per-cell sum in the same order as k_restrict: same bits.
+__device__ __forceinline__ int restrict_box_lo(int N) { return (N / 4) / 2; }
+__device__ __forceinline__ int restrict_box_hi(int N) { return (3 * (N / 4) + 1) / 2; }
+static __global__ void k_restrict_outer(int N, int L, const double *__restrict__ rho, double *__restrict__ rc)
+{
+    const int H = N / 2, lf = blockIdx.y + 1;                      // level lf projects onto level lf - 1
+    const size_t n3 = (size_t)N * N * N, h3 = n3 / 8;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= H * H * H) return;
+    const int ci = idx % H, cj = (idx / H) % H, ck = idx / (H * H), lo = restrict_box_lo(N), hi = restrict_box_hi(N);
+    if (lf < L - 1 && ci >= lo && ci < hi && cj >= lo && cj < hi && ck >= lo && ck < hi) return;   // the cascade's
+    // rho only: the two x-children of a parent are one aligned 16-byte word; summed in restrict_cell's order
+    const double *rho_f = rho + n3 * lf;
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int bb = 0; bb < 2; ++bb) {
+            const double2 v = __ldg(reinterpret_cast<const double2 *>(rho_f + ((size_t)(2 * ck + c) * N + (2 * cj + bb)) * N + 2 * ci));
+            s += v.x;
+            s += v.y;
+        }
+    rc[h3 * (lf - 1) + idx] = 0.125 * s;
+}
+static __global__ void k_restrict_inner(int N, int lf, const double *__restrict__ rho_f, const double *__restrict__ rc_f,
+                                        double *__restrict__ rc_out)
+{
+    const int H = N / 2, lo = restrict_box_lo(N), B = restrict_box_hi(N) - lo;
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= B * B * B) return;
+    const int ci = lo + idx % B, cj = lo + (idx / B) % B, ck = lo + idx / (B * B);
+    rc_out[((size_t)ck * H + cj) * H + ci] = restrict_cell(N, true, rho_f, rc_f, ci, cj, ck);
 }
 
 // Level sharding across GPUs: all that a8 of level b reads of level b-1 is H = ext + Phi_hole on the

@@ -216,11 +216,17 @@ int enqueue_solve(cm_plan *p, const double *rho, double *phi, cudaStream_t s, cu
     const size_t n3 = (size_t)N * N * N, h3 = (size_t)H * H * H;
     p->launches = 0;
     if (ev) cudaEventRecord(ev[0], s);
-    // a1: restriction cascade, fine -> coarse
-    for (int lf = L - 1; lf >= 1; --lf) {
-        const double *rc_f = (lf < L - 1) ? p->rc + h3 * lf : nullptr;
-        k_restrict<<<(unsigned)((h3 + 255) / 256), 256, 0, s>>>(N, lf, L, rho + n3 * lf, rc_f, p->rc + h3 * (lf - 1));
+    // a1: restriction cascade.  Every parent without a child under the next finer grid in one launch for all levels, then
+    // fine -> coarse the 1/8 of each level's parents that take already projected values (k_restrict_inner)
+    if (L > 1) {
+        k_restrict_outer<<<dim3((unsigned)((h3 + 255) / 256), L - 1), 256, 0, s>>>(N, L, rho, p->rc);
         p->launches++;
+        const int bx = (3 * (N / 4) + 1) / 2 - (N / 4) / 2;
+        for (int lf = L - 2; lf >= 1; --lf) {
+            k_restrict_inner<<<(unsigned)(((size_t)bx * bx * bx + 255) / 256), 256, 0, s>>>(N, lf, rho + n3 * lf, p->rc + h3 * lf,
+                                                                                             p->rc + h3 * (lf - 1));
+            p->launches++;
+        }
     }
     CM_CUDA(p, cudaGetLastError());
     if (ev) cudaEventRecord(ev[1], s);
