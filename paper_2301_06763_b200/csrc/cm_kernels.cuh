@@ -2,7 +2,7 @@
 //
 // Data flow of one solve (steps a1-a8 of SURVEY.md §8):
 //
-//   rho --k_restrict (fine->coarse cascade)--> rc        projected cavity density (L280-L282)
+//   rho --k_restrict* (fine->coarse cascade)--> rc       projected cavity density (L280-L282)
 //   per level b one COMPLEX field  c_b = rho_full + i rho_hole  (K-hat is real, so the
 //   real/imaginary parts of the convolution are Phi_full and Phi_hole: L174-L176)
 //   P1 k_x_fwd : rho,rc      -> W1[b][z<N][y<N][sx<2N]     x transform of [N data, N zeros]
