@@ -55,7 +55,7 @@ def _sharded(pkg, rho, N, L, dx0, G, world):
     return phi
 
 
-@pytest.mark.parametrize("N,L,world", [(32, 5, 1), (32, 5, 2), (32, 5, 3), (32, 5, 5), (32, 3, 5), (16, 2, 2), (20, 4, 2), (64, 4, 3),
+@pytest.mark.parametrize("N,L,world", [(32, 5, 1), (32, 5, 2), (32, 5, 3), (32, 5, 5), (32, 3, 5), (16, 2, 2), (16, 1, 1), (16, 1, 2), (20, 4, 2), (64, 4, 3),
                                        (128, 4, 3), (256, 2, 2)])
 def test_any_partition_of_the_levels_gives_the_bits_of_cm_potential(N, L, world):
     import paper_2301_06763_b200 as pkg
