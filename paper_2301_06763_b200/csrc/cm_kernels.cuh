@@ -175,7 +175,33 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
     double2 w[16];
     if (T > 1) {
         if (PRE) sync();
-        if constexpr (T <= 16) {
+        if constexpr (T <= 16 && DEC > 1) {
+            // Decimated: only the outputs jj = DEC jj' of the T-point stage are ever read (by the threads j % DEC == 0), and
+            //     y[DEC jj'] = sum_{m < T/DEC} ( sum_{q < DEC} V[m + (T/DEC) q] ) w_{T/DEC}^{m jj'}:
+            // fold the inputs (the K-hat product rides on the fold as FMAs), transform T/DEC points, write T/DEC columns.
+            constexpr int TD = T / DEC;
+#pragma unroll
+            for (int cc = 0; cc < 16 / T; ++cc) {
+                double2 f[TD];
+#pragma unroll
+                for (int m = 0; m < TD; ++m) {
+#pragma unroll
+                    for (int q = 0; q < DEC; ++q) {
+                        const int i = cc * T + m + TD * q;
+                        if (KM) {
+                            const double k = kh_at(kh, vslot<T>(i, j));
+                            f[m] = q ? make_double2(fma(k, v[i].x, f[m].x), fma(k, v[i].y, f[m].y)) : make_double2(k * v[i].x, k * v[i].y);
+                        } else {
+                            f[m] = q ? make_double2(f[m].x + v[i].x, f[m].y + v[i].y) : v[i];
+                        }
+                    }
+                }
+                Dft<TD, +1>::run(f);
+#pragma unroll
+                for (int jj = 0; jj < TD; ++jj) ex_at<Lay>(sm, cc * T + j, DEC * jj) = f[jj];
+            }
+            sync();
+        } else if constexpr (T <= 16) {
 #pragma unroll
             for (int cc = 0; cc < 16 / T; ++cc) {
                 if (KM) {
