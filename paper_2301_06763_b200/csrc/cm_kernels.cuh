@@ -162,6 +162,15 @@ __device__ __forceinline__ void fwd_half(const double2 (&a)[16], double2 (&v)[16
     }
 }
 
+// cos / sin of 2 pi n / 32, n = 0 .. 15 (the modulation of the odd half of a 32-point stage, folded variant)
+__host__ __device__ constexpr double cos32(int n)
+{
+    constexpr double t[9] = {1.0, 0.98078528040323043, 0.92387953251128674, 0.83146961230254524, 0.70710678118654757,
+                             0.55557023301960218, 0.38268343236508978, 0.19509032201612825, 0.0};
+    return n <= 8 ? t[n] : -t[16 - n];
+}
+__host__ __device__ constexpr double sin32(int n) { return n <= 8 ? cos32(8 - n) : cos32(n - 8); }
+
 // Inverse, parity P: v as above (consumed).  P = 0: on return o[r] is the even half's contribution to output
 // element n = j + T r, r < 16 (the cropped half).  P = 1: the odd half's contribution, times conj(w_32^r), is ADDED
 // to o[r] (the caller passes the even half's result).  KM: v is first multiplied by the real
@@ -220,6 +229,33 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
             // the 32-point stage backwards: thread (q, c) turns its outputs k2 = 2 m + q of row c into
             // y_q[jj] = w32^{-q jj} sum_m V[2m+q] w16^{-m jj}; the owner of column jj + 16 h then takes y_0 + (-1)^h y_1
             const int q = j >> 4, c = j & 15;
+            if constexpr (DEC > 1) {
+                // Decimated (see the T <= 16 branch): only the columns jj = DEC jj' are read, and for those
+                //     y_q[DEC jj'] = w32^{-q DEC jj'} sum_{m' < 16/DEC} ( sum_p V[2 (m' + (16/DEC) p) + q] ) w_{16/DEC}^{-m' jj'}
+                constexpr int TD = 16 / DEC;
+                double2 f[TD];
+#pragma unroll
+                for (int m = 0; m < TD; ++m) {
+#pragma unroll
+                    for (int p = 0; p < DEC; ++p) {
+                        const int i = m + TD * p;
+                        if (KM) {
+                            const double k = kh_at(kh, vslot<T>(i, j));
+                            f[m] = p ? make_double2(fma(k, v[i].x, f[m].x), fma(k, v[i].y, f[m].y)) : make_double2(k * v[i].x, k * v[i].y);
+                        } else {
+                            f[m] = p ? make_double2(f[m].x + v[i].x, f[m].y + v[i].y) : v[i];
+                        }
+                    }
+                }
+                Dft<TD, +1>::run(f);
+#pragma unroll
+                for (int jj = 0; jj < TD; ++jj) {
+                    // conj(w32)^{DEC jj}, applied by the odd-k2 thread only
+                    const double2 m32 = make_double2(cos32(DEC * jj), sin32(DEC * jj));
+                    ex_at<Lay>(sm, c, 16 * q + DEC * jj) = q ? cmul(f[jj], m32) : f[jj];
+                }
+                sync();
+            } else {
             double2 y[16];
             if (q) {
                 if (KM) {
@@ -248,6 +284,7 @@ __device__ __forceinline__ void inv_half(double2 (&v)[16], double2 (&o)[16], int
 #pragma unroll
             for (int jj = 0; jj < 16; ++jj) ex_at<Lay>(sm, c, 16 * q + jj) = y[jj];
             sync();
+            }
         }
         if (DEC > 1 && (j % DEC) != 0) return;
         TwCarry twc{make_double2(1.0, 0.0), make_double2(1.0, 0.0)};
