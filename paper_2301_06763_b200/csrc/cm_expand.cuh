@@ -138,7 +138,7 @@ __host__ __device__ __forceinline__ constexpr int freq_to_slot(int k, int N)   /
 template <int T, int DEC>
 __global__ void __launch_bounds__(batch_threads<T>(), 1)
 k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const double2 *__restrict__ tw,
-             const double2 *__restrict__ E, int zlo, int zhi, int b0, int L, int nd)
+             const double2 *__restrict__ E, int zlo, int zhi, int b0, int L, int nd, int ahead = 0)
 {
     using C = ZDecCfg<T>;
     constexpr int N = C::N, NN = C::NN, PEN = C::PEN, GX = NN / PEN;   // GX pencil groups per sy row
@@ -167,6 +167,33 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
             asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst + C::KE * 8),
                          "l"(ksrc + (size_t)q * C::RSK + N), "r"((N / 2) * 8), "r"(bar_k)
                          : "memory");
+        }
+    }
+    // One CTA (T = 32) or two per SM and loads straight into registers: nothing hides a tile's load latency (ncu, <32, 4>: fp64
+    // pipe 34 % busy, 20 % of the stall samples on the load scoreboard).  Pull into L2 what comes next: the rows of this CTA's
+    // mirror tile, and the first tile and the K-hat tile of the CTA `ahead` places later (the next one on this SM).
+    if (ahead > 0) {
+        auto pull_rows = [&](const double2 *c0) {      // one lane per 128-byte line of the rows this thread will load
+            if (px == 0) {
+#pragma unroll
+                for (int r = 0; r < 16; ++r) {
+                    const int z = j + T * r;
+                    if (z >= zlo && z < zhi) asm volatile("prefetch.global.L2 [%0];" ::"l"(c0 + (size_t)z * ZS));
+                }
+            }
+        };
+        const double2 *lvl = W2 + (size_t)b0 * nd * ZS;
+        if (ntile == 2) pull_rows(lvl + ((size_t)sy_b * NN + (size_t)gx * PEN + g * 8));
+        const unsigned nb = blockIdx.x + ahead;
+        if (nb < gridDim.x) {
+            const int sy2 = freq_to_slot((int)(nb / GX), N), gx2 = (int)(nb % GX);
+            pull_rows(lvl + ((size_t)sy2 * NN + (size_t)gx2 * PEN + g * 8));
+            const char *k2 = reinterpret_cast<const char *>(Kt + ((size_t)sy2 * NN + (size_t)gx2 * PEN) * C::RSK);
+            constexpr int LA = (C::KE * 8 + 127) / 128, LB = (N / 2 * 8 + 127) / 128;      // lines of the two stored halves
+            for (int i = tid; i < PEN * (LA + LB); i += batch_threads<T>()) {
+                const int q = i / (LA + LB), l = i % (LA + LB);
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(k2 + (size_t)q * C::RSK * 8 + (l < LA ? l * 128 : N * 8 + (l - LA) * 128)));
+            }
         }
     }
     // twiddles and E feed multiplies directly: from global memory their latency was 26 % of the warp time (ncu, T = 32)
