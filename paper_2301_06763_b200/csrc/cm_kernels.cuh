@@ -540,11 +540,13 @@ __device__ __forceinline__ void y_fwd_body(const double2 *src, double2 *dst, con
     }
 }
 
-template <int T, bool GEN = false>
+template <int T, bool GEN = false, bool PF = false>
 __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd(const double2 *__restrict__ W1, double2 *__restrict__ W2,
-                                                    const double2 *__restrict__ tw, int nd_arg = 0)
+                                                    const double2 *__restrict__ tw, int nd_arg = 0, int ahead = 0)
 {
     // GEN: a plane has nd <= N rows of data (see x_fwd_body); bz counts the nd planes of every level
+    // PF (one or two CTAs per SM and register loads: nothing else hides the load latency): pull the columns of the CTA `ahead`
+    // places later into L2.  A template flag: the code without it is untouched.
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     const int nd = GEN ? nd_arg : N;
     extern __shared__ double2 smem[];
@@ -552,6 +554,14 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd(const double2 *__r
     const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;      // (b*nd + z) * 2N + sx
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
+    if (PF && px == 0 && blockIdx.x + ahead < gridDim.x) {
+        const size_t q2 = (size_t)(blockIdx.x + ahead) * PEN + g * 8;
+        const double2 *s2 = W1 + (q2 / NN) * nd * NN + (q2 % NN);
+        const int j = (tid >> 3) % T;
+#pragma unroll
+        for (int r = 0; r < 16; ++r)
+            if (j + T * r < nd) asm volatile("prefetch.global.L2 [%0];" ::"l"(s2 + (size_t)(j + T * r) * NN));
+    }
     y_fwd_body<T>(W1 + bz * nd * NN + sx, W2 + bz * NN * NN + sx, tw, smem, 0, nd);
 }
 
@@ -600,11 +610,11 @@ __global__ void __launch_bounds__(2 * kThreads, 2) k_y_fwd_split(const double2 *
 }
 
 // ================================ P4: y inverse ====================================
-template <int T, bool GEN = false>
+template <int T, bool GEN = false, bool PF = false>
 __global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(const double2 *__restrict__ W2, double2 *__restrict__ W1,
-                                                    const double2 *__restrict__ tw, int nd_arg = 0)
+                                                    const double2 *__restrict__ tw, int nd_arg = 0, int ahead = 0)
 {
-    // GEN: only the nd <= N rows of data are kept (see x_fwd_body)
+    // GEN: only the nd <= N rows of data are kept (see x_fwd_body); ahead: as in k_y_fwd
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     const int nd = GEN ? nd_arg : N;
     using Lay = LayBatch<T>;
@@ -613,6 +623,15 @@ __global__ void __launch_bounds__(batch_threads<T>(), T == 32 ? 1 : 2) k_y_inv(c
     const size_t q = (size_t)blockIdx.x * PEN + g * 8 + px;
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
+    if (PF && px == 0 && blockIdx.x + ahead < gridDim.x) {
+        const size_t q2 = (size_t)(blockIdx.x + ahead) * PEN + g * 8;
+        const double2 *s2 = W2 + (q2 / NN) * NN * NN + (q2 % NN);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(s2 + (size_t)vslot<T>(i, j) * NN));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(s2 + (size_t)(N + vslot<T>(i, j)) * NN));
+        }
+    }
     const double2 *src = W2 + bz * NN * NN + sx;
     double2 *dst = W1 + bz * nd * NN + sx;
     double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;

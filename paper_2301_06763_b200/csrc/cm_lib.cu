@@ -14,6 +14,8 @@ template <int T> int set_attrs(cm_plan *p)
     CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute((k_y_fwd<T, false, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+    CM_CUDA(p, cudaFuncSetAttribute((k_y_inv<T, false, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     if constexpr (T >= 2) {     // general sizes (N < 16 T)
         CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
         CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
@@ -52,7 +54,7 @@ template <int T> void launch_zconv(cm_plan *p, cudaStream_t s, int b0, int L)
         // N = 512: the batch-fastest P3 of cm_expand.cuh without decimation (a CTA per (|f_y|, 8 pencils): K-hat tile shared
         // by the two mirror tiles and by the levels)
         k_z_conv_dec<T, 1><<<(unsigned)((size_t)(N + 1) * (NN / batch_pencils<T>())), batch_threads<T>(), ZDecCfg<T>::SMEM, s>>>(
-            p->Khat, p->W2, p->tw, nullptr, 0, p->N, b0, L, p->N);
+            p->Khat, p->W2, p->tw, nullptr, 0, p->N, b0, L, p->N, /*ahead=*/p->num_sms);
     }
 }
 
@@ -92,6 +94,10 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     const double scale0 = -p->G * p->dx0 * p->dx0;
     const unsigned gx = (unsigned)((rows + ROWS - 1) / ROWS), gy = (unsigned)(planes * NN / PEN);
     bool done_x = false, done_y = false;
+    // L2 prefetch of the columns of the CTA half a wave (N = 128) or a wave (N = 512: one CTA per SM) ahead in P2 / P4 — measured
+    // per size (profiles/r02_pass_variants.md): -10 % / -3 % at N = 128, -16 % / -11 % at N = 512, nothing at N = 256 (P4 is at the
+    // copy peak there and P2 is the split kernel with its own prefetch) and at N <= 64 (L2-resident)
+    const int ya = (T == 32 || T == 8) ? p->num_sms : 0, ya4 = ya;
     if constexpr (T <= 16) {
         if (p->split_x) {
             k_x_fwd_split<T><<<gx, 2 * kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, L);
@@ -111,12 +117,14 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
     }
     if (!done_y) {
         if (p->gen) k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, nd);
+        else if (ya > 0) k_y_fwd<T, false, true><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, 0, ya);
         else k_y_fwd<T, false><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     }
     if (ev) cudaEventRecord(ev[3], s);
     launch_zconv<T>(p, s, 0, L);
     if (ev) cudaEventRecord(ev[4], s);
     if (p->gen) k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw, nd);
+    else if (ya4 > 0) k_y_inv<T, false, true><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw, 0, ya4);
     else k_y_inv<T, false><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
     if (ev) cudaEventRecord(ev[5], s);
     const size_t lrows = (size_t)nd * nd;
