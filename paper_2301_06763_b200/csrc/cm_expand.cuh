@@ -83,7 +83,7 @@ __global__ void __launch_bounds__(kThreads) k_x_fwd_blk(const double *__restrict
 // P2 on the block's z-planes: plane zc -> z = c0 + zc; rows outside [c0, c0 + Nc) are zero and not read.
 template <int T>
 __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd_blk(const double2 *__restrict__ W1, double2 *__restrict__ W2,
-                                                                  const double2 *__restrict__ tw, int Nc, int c0)
+                                                                  const double2 *__restrict__ tw, int Nc, int c0, int ahead = 0)
 {
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     extern __shared__ double2 smem[];
@@ -92,6 +92,16 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_fwd_blk(const double2 
     const size_t z = c0 + q / NN;
     const int sx = (int)(q % NN);
     const size_t nbig = 2 * (size_t)c0 + Nc;       // rows per plane of the expanded grid as W1 holds it
+    if (ahead > 0 && px == 0 && blockIdx.x + ahead < gridDim.x) {     // the next resident CTA's columns into L2 (see k_y_fwd)
+        const size_t q2 = (size_t)(blockIdx.x + ahead) * PEN + g * 8;
+        const double2 *s2 = W1 + (c0 + q2 / NN) * nbig * NN + (q2 % NN);
+        const int j = (tid >> 3) % T;
+#pragma unroll
+        for (int r = 0; r < 16; ++r) {
+            const int y = j + T * r;
+            if (y >= c0 && y < c0 + Nc) asm volatile("prefetch.global.L2 [%0];" ::"l"(s2 + (size_t)y * NN));
+        }
+    }
     y_fwd_body<T>(W1 + z * nbig * NN + sx, W2 + z * NN * NN + sx, tw, smem, c0, c0 + Nc);
 }
 
@@ -238,7 +248,8 @@ k_z_conv_dec(const double *__restrict__ Kt, double2 *__restrict__ W2, const doub
 // P4, decimated: plane bz = coarse z; the N / DEC coarse rows a = (j + T r) / DEC of W1 (plane stride as in the plain pass).
 template <int T, int DEC>
 __global__ void __launch_bounds__(batch_threads<T>()) k_y_inv_dec(const double2 *__restrict__ W2, double2 *__restrict__ W1,
-                                                                  const double2 *__restrict__ tw, const double2 *__restrict__ E, int Nc)
+                                                                  const double2 *__restrict__ tw, const double2 *__restrict__ E, int Nc,
+                                                                  int ahead = 0)
 {
     constexpr int N = 16 * T, NN = 2 * N, PEN = batch_pencils<T>();
     using Lay = LayBatch<T>;
@@ -248,6 +259,15 @@ __global__ void __launch_bounds__(batch_threads<T>()) k_y_inv_dec(const double2 
     const size_t bz = q / NN;
     const int sx = (int)(q % NN);
     const double2 *src = W2 + bz * NN * NN + sx;
+    if (ahead > 0 && px == 0 && blockIdx.x + ahead < gridDim.x) {     // the next resident CTA's columns into L2 (see k_y_fwd)
+        const size_t q2 = (size_t)(blockIdx.x + ahead) * PEN + g * 8;
+        const double2 *s2 = W2 + (q2 / NN) * NN * NN + (q2 % NN);
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(s2 + (size_t)vslot<T>(i, j) * NN));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(s2 + (size_t)(N + vslot<T>(i, j)) * NN));
+        }
+    }
     double2 *dst = W1 + bz * N * NN + sx;
     double2 *bufA = smem + (g * 8 + px) * Lay::PS, *bufB = bufA + PEN * Lay::PS;
     double2 v0[16], v1[16], e[16];

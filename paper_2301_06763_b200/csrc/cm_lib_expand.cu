@@ -28,11 +28,12 @@ template <int T, int F> int expanded_passes(cm_plan *pe, const double *src_re, c
     // the expanded grid has pe->N = F Nc cells per axis (transformed at N = 16 T >= pe->N); the block sits in its middle
     const int Nc = pe->N / F, c0 = (pe->N - Nc) / 2;
     const unsigned gr = (unsigned)(((size_t)Nc * Nc + ROWS - 1) / ROWS);
+    const int ya = pe->num_sms;   // y passes: L2 prefetch distance in CTAs (measured 74 ... 148 equal, 296 no gain)
     k_x_fwd_blk<T><<<gr, kThreads, smem_row<T>(), s>>>(src_re, src_im, pe->W1, pe->tw, Nc, c0);
-    k_y_fwd_blk<T><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W1, pe->W2, pe->tw, Nc, c0);
+    k_y_fwd_blk<T><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W1, pe->W2, pe->tw, Nc, c0, ya);
     k_z_conv_dec<T, F><<<(unsigned)((size_t)(N + 1) * (NN / PEN)), BT, ZDecCfg<T>::SMEM, s>>>(pe->Khat, pe->W2, pe->tw, pe->decE, c0, c0 + Nc, 0, 1, 0,
                                                                                                         /*ahead=*/(T == 32 ? 1 : 2) * pe->num_sms);
-    k_y_inv_dec<T, F><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W2, pe->W1, pe->tw, pe->decE, Nc);
+    k_y_inv_dec<T, F><<<(unsigned)((size_t)Nc * NN / PEN), BT, smem_batch<T>(), s>>>(pe->W2, pe->W1, pe->tw, pe->decE, Nc, ya);
     k_x_inv_dec<T, F><<<gr, kThreads, smem_row<T>(), s>>>(pe->W1, out_re, out_im, pe->tw, pe->decE, -1.0, Nc);
     CM_CUDA(pe, cudaGetLastError());
     return CM_OK;
