@@ -21,6 +21,8 @@ template <int T> int set_attrs(cm_plan *p)
         CM_CUDA(p, cudaFuncSetAttribute(k_x_inv<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
         CM_CUDA(p, cudaFuncSetAttribute(k_y_fwd<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
         CM_CUDA(p, cudaFuncSetAttribute(k_y_inv<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute((k_y_fwd<T, true, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
+        CM_CUDA(p, cudaFuncSetAttribute((k_y_inv<T, true, true>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_batch<T>()));
     }
     if constexpr (T <= 16) {
         CM_CUDA(p, cudaFuncSetAttribute(k_x_fwd_split<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_row<T>()));
@@ -116,14 +118,16 @@ template <int T> int launch_passes(cm_plan *p, const double *rho, double *phi, c
         }
     }
     if (!done_y) {
-        if (p->gen) k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, nd);
+        if (p->gen && ya > 0) k_y_fwd<T, true, true><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, nd, ya);
+        else if (p->gen) k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, nd);
         else if (ya > 0) k_y_fwd<T, false, true><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw, 0, ya);
         else k_y_fwd<T, false><<<gy, BT, smem_batch<T>(), s>>>(p->W1, p->W2, p->tw);
     }
     if (ev) cudaEventRecord(ev[3], s);
     launch_zconv<T>(p, s, 0, L);
     if (ev) cudaEventRecord(ev[4], s);
-    if (p->gen) k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw, nd);
+    if (p->gen && ya4 > 0) k_y_inv<T, true, true><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw, nd, ya4);
+    else if (p->gen) k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw, nd);
     else if (ya4 > 0) k_y_inv<T, false, true><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw, 0, ya4);
     else k_y_inv<T, false><<<gy, BT, smem_batch<T>(), s>>>(p->W2, p->W1, p->tw);
     if (ev) cudaEventRecord(ev[5], s);
@@ -185,16 +189,21 @@ template <int T> void range_p1_to_p4(cm_plan *p, const double *rho, cudaStream_t
     const size_t lrows = (size_t)nd * nd;
     double2 *w1 = p->W1 + (size_t)lo * lrows * NN, *w2 = p->W2 + (size_t)lo * nd * NN * NN;
     const unsigned gx = (unsigned)((nl * lrows + ROWS - 1) / ROWS), gy = (unsigned)((size_t)nl * nd * NN / PEN);
+    const int ya = (T == 32 || T == 8) ? p->num_sms : 0;      // as in launch_passes
     if (p->gen) {
         k_x_fwd<T, true><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)lo * lrows, nd, (size_t)hi * lrows);
-        k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw, nd);
+        if (ya > 0) k_y_fwd<T, true, true><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw, nd, ya);
+        else k_y_fwd<T, true><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw, nd);
         launch_zconv<T>(p, s, lo, nl);
-        k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw, nd);
+        if (ya > 0) k_y_inv<T, true, true><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw, nd, ya);
+        else k_y_inv<T, true><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw, nd);
     } else {
         k_x_fwd<T, false><<<gx, kThreads, smem_row<T>(), s>>>(rho, p->rc, p->W1, p->tw, p->L, (size_t)lo * lrows);
-        k_y_fwd<T, false><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw);
+        if (ya > 0) k_y_fwd<T, false, true><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw, 0, ya);
+        else k_y_fwd<T, false><<<gy, BT, smem_batch<T>(), s>>>(w1, w2, p->tw);
         launch_zconv<T>(p, s, lo, nl);
-        k_y_inv<T, false><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw);
+        if (ya > 0) k_y_inv<T, false, true><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw, 0, ya);
+        else k_y_inv<T, false><<<gy, BT, smem_batch<T>(), s>>>(w2, w1, p->tw);
     }
 }
 template <int T> void range_p5(cm_plan *p, double *phi, cudaStream_t s, int lo, int hi)
